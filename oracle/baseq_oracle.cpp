@@ -1,0 +1,258 @@
+// BASE-Q W4A4 linear hot path -- CPU ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT.
+//
+// Plain, slow, single-threaded C++17 restatement of what the hot path computes,
+// written from PAPER.md (arxiv 2506.15689) and the readings C-1..C-15 recorded in
+// DESIGN.md.  It shares no code, header, table or helper with the CUDA path
+// (paper_2506_15689_b200/csrc) and must never be imported, linked or executed by the
+// product: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may call it.
+//
+// Build: g++ -std=c++17 -O2 -ffp-contract=off -fno-fast-math -shared -fPIC
+// (no -march flags: every fp32 line below must be one correctly rounded IEEE op;
+//  -ffp-contract=off forbids the compiler from fusing a*b+c on its own).
+//
+// Citation convention: P:n = /root/reference/PAPER.md line n, S:n = SPEC.md line n.
+//
+// Parity status of each function (see tests/test_oracle_pins.py):
+//   oracle_hadamard_blocks   pinned (dense +-1 matrix product on integer inputs, H*H = I,
+//                            one-hot -> a/sqrt(B), Eq. 2)
+//   oracle_quantize_act      pinned (reduces to independent RTN, lattice rows, tie rule,
+//                            clip, reconstruction bound, s^2/12 law P:79, bias-correction
+//                            variance identity Eq. 6)
+//   oracle_gemm_i32          pinned (closed forms, one-hot rows, K-permutation invariance,
+//                            numpy int64 matmul on small shapes)
+//   oracle_epilogue          pinned (hand case, Eq. 14 cancellation P:222, exact
+//                            rational arithmetic via Python fractions)
+//   oracle_fused_bias        pinned to <= 1 fp32 ulp of an exact-rational recomputation;
+//                            bit-level summation order is this file's choice
+//                            ("parity unpinned at bit level" -- the GPU packer is compared
+//                            to it with the same 1-ulp bound, and GEMM parity runs feed
+//                            both sides the same fb)
+//   oracle_bf16_from_double  pinned (exhaustive vs exact-rational rounding on samples,
+//                            ties, subnormals)
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+// bf16 -> fp32 is exact: bf16 is the top 16 bits of an IEEE binary32.
+inline float bf16_bits_to_float(uint16_t h) {
+  uint32_t u = static_cast<uint32_t>(h) << 16;
+  float f;
+  std::memcpy(&f, &u, sizeof f);
+  return f;
+}
+
+// Sign-extend a two's-complement nibble (D2 in SURVEY: code q in [-8,7] stored as q & 0xF).
+inline int nibble_to_int(unsigned v) {
+  v &= 0xFu;
+  return (v >= 8u) ? static_cast<int>(v) - 16 : static_cast<int>(v);
+}
+
+}  // namespace
+
+extern "C" {
+
+// ---------------------------------------------------------------------------------------
+// Round a double to bfloat16 with ONE rounding (round-half-to-even), returned as the 16
+// bit pattern.  bf16 = 1 sign, 8 exponent, 7 fraction bits; same exponent range as fp32
+// (normal from 2^-126, subnormal quantum 2^-133).  Written from the definition: scale
+// the value so that one bf16 ulp becomes 1.0, round to integer with nearbyint (default
+// rounding mode = RNE), scale back.  Every scaling is by a power of two and therefore
+// exact in fp64.
+// ---------------------------------------------------------------------------------------
+uint16_t oracle_bf16_from_double(double y) {
+  if (std::isnan(y)) return 0x7FC0;
+  uint16_t sign = std::signbit(y) ? 0x8000u : 0u;
+  double a = std::fabs(y);
+  if (a == 0.0) return sign;
+  if (std::isinf(a)) return static_cast<uint16_t>(sign | 0x7F80u);
+  int e;
+  (void)std::frexp(a, &e);              // a = m * 2^e, m in [0.5, 1)  ->  2^(e-1) <= a < 2^e
+  int ulp_exp = (e - 1) - 7;            // exponent of one bf16 ulp for a normal number
+  if (ulp_exp < -133) ulp_exp = -133;   // subnormal range: fixed quantum 2^-133
+  double q = std::nearbyint(std::ldexp(a, -ulp_exp));   // integer number of ulps, RNE
+  double r = std::ldexp(q, ulp_exp);                    // exactly representable in bf16 (or overflow)
+  if (r >= std::ldexp(1.0, 128)) return static_cast<uint16_t>(sign | 0x7F80u);  // rounds to inf
+  float f = static_cast<float>(r);      // exact: r has <= 8 significant bits
+  uint32_t u;
+  std::memcpy(&u, &f, sizeof u);
+  return static_cast<uint16_t>(sign | (u >> 16));
+}
+
+// ---------------------------------------------------------------------------------------
+// Q1 (reading C-11): block-diagonal Hadamard, Sylvester order, fp32.
+// For each aligned block of B channels: in-place butterflies with increasing stride
+//   for h = 1, 2, 4, ..., B/2: for each i with (i & h) == 0: (a, b) <- (a + b, a - b)
+// then every element is multiplied once by c = (float)(1/sqrt((double)B)).
+// Eq. 2: "orthogonal Hadamard rotation H (where each entry is +-n^{-1/2})";
+// R^{-1} is applied before s^a and b^c in Eq. 15 P:228.  FWHT definition S:135-143.
+// ---------------------------------------------------------------------------------------
+void oracle_hadamard_blocks(float* x, int n, int B) {
+  const float c = static_cast<float>(1.0 / std::sqrt(static_cast<double>(B)));
+  for (int base = 0; base < n; base += B) {
+    float* v = x + base;
+    for (int h = 1; h < B; h <<= 1) {
+      for (int i = 0; i < B; ++i) {
+        if ((i & h) == 0) {
+          float a = v[i];
+          float b = v[i + h];
+          v[i] = a + b;
+          v[i + h] = a - b;
+        }
+      }
+    }
+    for (int i = 0; i < B; ++i) v[i] = v[i] * c;
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// The activation quantizer, steps Q0..Q7 of DESIGN.md (one correctly rounded fp32 op per
+// line).  Eq. 15:  Q_a( s^a R^{-1} s^{-1} x - b^c )  -- scale first, then subtract
+// (reading C-1); per-token dynamic SYMMETRIC int4 (north_star; P:241 for "per-token
+// dynamic"; reading C-4); clip ratio alpha multiplies the per-token absmax (P:231, S:208,
+// reading C-8); scale divisor 7, clamp range [-8, 7] (reading C-7);
+// round-half-to-even (north_star, reading C-6); floor 1e-12 (reading C-10);
+// one reciprocal per row and one multiply per element (reading C-5).
+//
+//   x_bf16 : [T, ldx] bf16 bit patterns, row-major, first K of each row used
+//   sa     : [K] per-channel s^a (already divided by the paired scale s), or NULL -> gamma
+//   b      : [K] correction bias b^c in the scaled domain, or NULL -> 0
+//   codes  : [T, K/2] bytes, byte j = (q[2j] & 15) | ((q[2j+1] & 15) << 4)
+//   scales : [T] fp32 per-token step size s_t
+//   u_out  : optional [T, K] fp32 dump of the pre-quantization values u (tests only)
+// Returns 0 on success, nonzero on invalid arguments (empty input S:57/S:225, alpha range
+// S:208-211, non-power-of-two Hadamard block S:139).
+// ---------------------------------------------------------------------------------------
+int oracle_quantize_act(const uint16_t* x_bf16, int64_t ldx, int T, int K, float alpha,
+                        float gamma, const float* sa, const float* b, int had_block,
+                        uint8_t* codes, float* scales, float* u_out) {
+  if (T < 1 || K < 2 || (K & 1)) return 2;
+  if (!(alpha > 0.0f) || !(alpha <= 1.0f)) return 4;
+  if (had_block != 0) {
+    if (had_block < 2 || (had_block & (had_block - 1)) != 0 || K % had_block != 0) return 4;
+  }
+  std::vector<float> x(static_cast<size_t>(K));
+  std::vector<float> u(static_cast<size_t>(K));
+  for (int t = 0; t < T; ++t) {
+    // Q0: exact widening of the stored bf16 activations (D1).
+    for (int k = 0; k < K; ++k) x[k] = bf16_bits_to_float(x_bf16[static_cast<int64_t>(t) * ldx + k]);
+    // Q1: optional online block Hadamard R^{-1}.
+    if (had_block) oracle_hadamard_blocks(x.data(), K, had_block);
+    // Q2: u_k = fma(g_k, x_k, -b_k)   (Eq. 15; a single rounding).
+    for (int k = 0; k < K; ++k) {
+      float g = sa ? sa[k] : gamma;
+      float bk = b ? b[k] : 0.0f;
+      u[k] = std::fmaf(g, x[k], -bk);
+    }
+    // Q3: per-token absmax (exact, order-free).
+    float m = 0.0f;
+    for (int k = 0; k < K; ++k) m = std::fmax(m, std::fabs(u[k]));
+    // Q4: s_t = max((alpha * m) / 7, 1e-12)  -- multiply, then divide, then max.
+    float am = alpha * m;
+    float st = am / 7.0f;
+    st = std::fmax(st, 1e-12f);
+    // Q5: one reciprocal per row.
+    float inv = 1.0f / st;
+    // Q6: r = u * inv; q = clamp(rint(r), -8, 7)   (Eq. 4: clip o round).
+    // Q7: pack two's-complement nibbles, low nibble = even k.
+    for (int k = 0; k < K; k += 2) {
+      int q2[2];
+      for (int j = 0; j < 2; ++j) {
+        float r = u[k + j] * inv;
+        float rr = std::nearbyintf(r);       // default rounding mode: ties to even
+        if (rr < -8.0f) rr = -8.0f;
+        if (rr > 7.0f) rr = 7.0f;
+        q2[j] = static_cast<int>(rr);
+      }
+      codes[static_cast<int64_t>(t) * (K / 2) + k / 2] =
+          static_cast<uint8_t>((q2[0] & 0xF) | ((q2[1] & 0xF) << 4));
+    }
+    scales[t] = st;
+    if (u_out) std::memcpy(u_out + static_cast<int64_t>(t) * K, u.data(), sizeof(float) * K);
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------
+// Fused bias  fb[n] = s_w[n] * sum_k qw[n,k] * b[k] + bias[n]   ("fused bias" WRb^c + b of
+// Eq. 14; reading C-3: W there is the DEQUANTISED int4 weight the GEMM multiplies, so
+// that W(x - b) + Wb = Wx cancels exactly).  fp64 accumulation, k ascending, rounded once
+// to fp32 at the end.
+// ---------------------------------------------------------------------------------------
+int oracle_fused_bias(const uint8_t* w_nibbles, const float* w_scale, const float* b,
+                      const float* layer_bias, int N, int K, float* fb) {
+  if (N < 1 || K < 2 || (K & 1)) return 2;
+  for (int n = 0; n < N; ++n) {
+    double s = 0.0;
+    if (b) {
+      for (int k = 0; k < K; ++k) {
+        unsigned byte = w_nibbles[static_cast<int64_t>(n) * (K / 2) + k / 2];
+        int q = nibble_to_int((k & 1) ? (byte >> 4) : byte);
+        s += static_cast<double>(q) * static_cast<double>(b[k]);
+      }
+    }
+    double v = static_cast<double>(w_scale[n]) * s;
+    if (layer_bias) v += static_cast<double>(layer_bias[n]);
+    fb[n] = static_cast<float>(v);
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------
+// Integer GEMM  acc[t,n] = sum_k qa[t,k] * qw[n,k]  in int32 ("4-bit matrix
+// multiplications"; exact: |acc| <= 64 * K).  Three nested loops over unpacked nibbles.
+// ---------------------------------------------------------------------------------------
+int oracle_gemm_i32(const uint8_t* codes, const uint8_t* w_nibbles, int T, int N, int K,
+                    int32_t* acc) {
+  if (T < 1 || N < 1 || K < 2 || (K & 1)) return 2;
+  std::vector<int8_t> qa(static_cast<size_t>(T) * K);
+  std::vector<int8_t> qw(static_cast<size_t>(N) * K);
+  for (int64_t i = 0; i < static_cast<int64_t>(T) * (K / 2); ++i) {
+    qa[2 * i] = static_cast<int8_t>(nibble_to_int(codes[i]));
+    qa[2 * i + 1] = static_cast<int8_t>(nibble_to_int(codes[i] >> 4));
+  }
+  for (int64_t i = 0; i < static_cast<int64_t>(N) * (K / 2); ++i) {
+    qw[2 * i] = static_cast<int8_t>(nibble_to_int(w_nibbles[i]));
+    qw[2 * i + 1] = static_cast<int8_t>(nibble_to_int(w_nibbles[i] >> 4));
+  }
+  for (int t = 0; t < T; ++t) {
+    const int8_t* a = qa.data() + static_cast<size_t>(t) * K;
+    for (int n = 0; n < N; ++n) {
+      const int8_t* w = qw.data() + static_cast<size_t>(n) * K;
+      int32_t s = 0;
+      for (int k = 0; k < K; ++k) s += static_cast<int32_t>(a[k]) * static_cast<int32_t>(w[k]);
+      acc[static_cast<int64_t>(t) * N + n] = s;
+    }
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------
+// Dequant epilogue (K3 in SURVEY; "fuse the online bias and scaling ... within
+// quantization and de-quantization"):  y = (s_t * s_w[n]) * acc + fb[n], in fp64:
+//   p   = (double)s_t * (double)s_w[n]       (exact: 24 x 24 bit product)
+//   y64 = fma(p, (double)acc, (double)fb[n]) (one rounding)
+//   Y   = bf16_rne(y64)                      (one rounding; reading C-9)
+// y64_out (optional) receives the unrounded fp64 values.
+// ---------------------------------------------------------------------------------------
+int oracle_epilogue(const int32_t* acc, const float* scales, const float* w_scale,
+                    const float* fb, int T, int N, uint16_t* y_bf16, double* y64_out) {
+  if (T < 1 || N < 1) return 2;
+  for (int t = 0; t < T; ++t) {
+    for (int n = 0; n < N; ++n) {
+      double p = static_cast<double>(scales[t]) * static_cast<double>(w_scale[n]);
+      double f = fb ? static_cast<double>(fb[n]) : 0.0;
+      double y = std::fma(p, static_cast<double>(acc[static_cast<int64_t>(t) * N + n]), f);
+      if (y64_out) y64_out[static_cast<int64_t>(t) * N + n] = y;
+      y_bf16[static_cast<int64_t>(t) * N + n] = oracle_bf16_from_double(y);
+    }
+  }
+  return 0;
+}
+
+int oracle_version(void) { return 1; }
+
+}  // extern "C"

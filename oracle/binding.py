@@ -1,0 +1,155 @@
+"""ctypes marshalling for oracle/baseq_oracle.cpp.  TEST INFRASTRUCTURE, NOT PRODUCT.
+
+No arithmetic of the method lives here: every function checks dtypes/shapes, allocates
+numpy outputs and calls the C++ routine of the same name.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "baseq_oracle.cpp")
+_LIB = os.path.join(_HERE, "libbaseq_oracle.so")
+_lib = None
+
+# -ffp-contract=off: the compiler must not fuse a*b+c; no -march/-ffast-math: every fp32
+# line of the oracle is one correctly rounded IEEE operation (oracle contract).
+_CXXFLAGS = ["-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
+
+
+def build(force=False):
+    """Compile the oracle with g++ (no CUDA).  Returns the path of the shared object."""
+    if force or (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["g++", *_CXXFLAGS, _SRC, "-o", tmp])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        c = ctypes
+        lib.oracle_bf16_from_double.restype = c.c_uint16
+        lib.oracle_bf16_from_double.argtypes = [c.c_double]
+        lib.oracle_hadamard_blocks.restype = None
+        lib.oracle_hadamard_blocks.argtypes = [c.c_void_p, c.c_int, c.c_int]
+        lib.oracle_quantize_act.restype = c.c_int
+        lib.oracle_quantize_act.argtypes = [c.c_void_p, c.c_int64, c.c_int, c.c_int, c.c_float,
+                                            c.c_float, c.c_void_p, c.c_void_p, c.c_int,
+                                            c.c_void_p, c.c_void_p, c.c_void_p]
+        lib.oracle_fused_bias.restype = c.c_int
+        lib.oracle_fused_bias.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                                          c.c_int, c.c_int, c.c_void_p]
+        lib.oracle_gemm_i32.restype = c.c_int
+        lib.oracle_gemm_i32.argtypes = [c.c_void_p, c.c_void_p, c.c_int, c.c_int, c.c_int,
+                                        c.c_void_p]
+        lib.oracle_epilogue.restype = c.c_int
+        lib.oracle_epilogue.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                                        c.c_int, c.c_int, c.c_void_p, c.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _chk(a, dtype, name):
+    if a is None:
+        return None
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags.c_contiguous:
+        raise TypeError("%s must be a C-contiguous numpy array of %s" % (name, np.dtype(dtype)))
+    return a
+
+
+def bf16_from_double(y):
+    """bf16 bit pattern (int) of a Python float, one RNE rounding."""
+    return int(_load().oracle_bf16_from_double(float(y)))
+
+
+def hadamard_blocks(x, block):
+    """In-place fp32 block Hadamard of a 1-D float32 array (Q1)."""
+    _chk(x, np.float32, "x")
+    if x.ndim != 1 or x.size % block:
+        raise ValueError("x must be 1-D with length a multiple of block")
+    _load().oracle_hadamard_blocks(_ptr(x), x.size, block)
+    return x
+
+
+def quantize_act(x_bf16, alpha, gamma=1.0, sa=None, b=None, had_block=0, return_u=False):
+    """x_bf16: [T,K] uint16 bf16 bit patterns.  Returns (codes [T,K/2] u8, scales [T] f32[, u])."""
+    _chk(x_bf16, np.uint16, "x_bf16")
+    if x_bf16.ndim != 2:
+        raise ValueError("x_bf16 must be [T,K]")
+    T, K = x_bf16.shape
+    _chk(sa, np.float32, "sa")
+    _chk(b, np.float32, "b")
+    for v, n in ((sa, "sa"), (b, "b")):
+        if v is not None and v.shape != (K,):
+            raise ValueError("%s must have shape [K]" % n)
+    codes = np.empty((T, max(K // 2, 0)), dtype=np.uint8)
+    scales = np.empty((T,), dtype=np.float32)
+    u = np.empty((T, K), dtype=np.float32) if return_u else None
+    rc = _load().oracle_quantize_act(_ptr(x_bf16), K, T, K, alpha, gamma, _ptr(sa), _ptr(b),
+                                     had_block, _ptr(codes), _ptr(scales), _ptr(u))
+    if rc:
+        raise ValueError("oracle_quantize_act: invalid arguments (status %d)" % rc)
+    return (codes, scales, u) if return_u else (codes, scales)
+
+
+def fused_bias(w_nibbles, w_scale, b=None, layer_bias=None):
+    """fb[n] = s_w[n] * sum_k qw[n,k] b[k] + bias[n]  (fp64 accumulate, fp32 result)."""
+    _chk(w_nibbles, np.uint8, "w_nibbles")
+    _chk(w_scale, np.float32, "w_scale")
+    _chk(b, np.float32, "b")
+    _chk(layer_bias, np.float32, "layer_bias")
+    N, Kh = w_nibbles.shape
+    fb = np.empty((N,), dtype=np.float32)
+    rc = _load().oracle_fused_bias(_ptr(w_nibbles), _ptr(w_scale), _ptr(b), _ptr(layer_bias),
+                                   N, 2 * Kh, _ptr(fb))
+    if rc:
+        raise ValueError("oracle_fused_bias: invalid arguments (status %d)" % rc)
+    return fb
+
+
+def gemm_i32(codes, w_nibbles):
+    """acc[t,n] = sum_k qa[t,k] qw[n,k], int32, triple loop."""
+    _chk(codes, np.uint8, "codes")
+    _chk(w_nibbles, np.uint8, "w_nibbles")
+    T, Kh = codes.shape
+    N, Kh2 = w_nibbles.shape
+    if Kh != Kh2:
+        raise ValueError("K mismatch")
+    acc = np.empty((T, N), dtype=np.int32)
+    rc = _load().oracle_gemm_i32(_ptr(codes), _ptr(w_nibbles), T, N, 2 * Kh, _ptr(acc))
+    if rc:
+        raise ValueError("oracle_gemm_i32: invalid arguments (status %d)" % rc)
+    return acc
+
+
+def epilogue(acc, scales, w_scale, fb=None, return_y64=False):
+    """Y = bf16_rne(fma(s_t*s_w[n], acc, fb[n])) in fp64.  Returns uint16 [T,N] (and y64)."""
+    _chk(acc, np.int32, "acc")
+    _chk(scales, np.float32, "scales")
+    _chk(w_scale, np.float32, "w_scale")
+    _chk(fb, np.float32, "fb")
+    T, N = acc.shape
+    y = np.empty((T, N), dtype=np.uint16)
+    y64 = np.empty((T, N), dtype=np.float64) if return_y64 else None
+    rc = _load().oracle_epilogue(_ptr(acc), _ptr(scales), _ptr(w_scale), _ptr(fb), T, N,
+                                 _ptr(y), _ptr(y64))
+    if rc:
+        raise ValueError("oracle_epilogue: invalid arguments (status %d)" % rc)
+    return (y, y64) if return_y64 else y
+
+
+def linear(x_bf16, w_nibbles, w_scale, fb, alpha, gamma=1.0, sa=None, b=None, had_block=0):
+    """quantize_act -> gemm_i32 -> epilogue.  Returns dict(codes, scales, acc, y, y64)."""
+    codes, scales = quantize_act(x_bf16, alpha, gamma, sa, b, had_block)
+    acc = gemm_i32(codes, w_nibbles)
+    y, y64 = epilogue(acc, scales, w_scale, fb, return_y64=True)
+    return {"codes": codes, "scales": scales, "acc": acc, "y": y, "y64": y64}
