@@ -1,0 +1,146 @@
+/* libbaseq -- C ABI of the BASE-Q W4A4 linear hot path for NVIDIA B200 (sm_100a).
+ *
+ * The operation is the online quantised linear layer of BASE-Q (arxiv 2506.15689):
+ *
+ *   Y = Q_w(W s R) . Q_a( s^a R^-1 s^-1 x - b^c ) + (W R b^c + b)          (Eq. 15)
+ *
+ * split the way the paper deploys it (Fig. 6): a fused quantisation kernel
+ * (online Hadamard, scale, bias, per-token int4), an int4 x int4 -> int32 GEMM, and a fused
+ * de-quantisation (both scales + fused bias).  P:n below = PAPER.md line n, S:n = SPEC.md
+ * line n, C-n = the readings listed in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *  - plain C, no torch / C++ types; every pointer is a DEVICE pointer owned by the caller
+ *    unless the argument name ends in _host;
+ *  - the library never allocates, frees or synchronises, and keeps no reference to any
+ *    argument after the call returns; all work is enqueued on `stream` (a cudaStream_t
+ *    passed as void*; NULL = the legacy default stream);
+ *  - arguments are validated on the host before anything is launched; every call returns a
+ *    baseq_status_t (no exceptions, no errno, nothing printed);
+ *  - there is no CPU fallback: on a device that is not compute capability 10.x every compute
+ *    entry point returns BASEQ_ERR_UNSUPPORTED;
+ *  - CUDA launch failures are returned as BASEQ_ERR_CUDA by the enqueueing call;
+ *    asynchronous faults surface at the caller's next synchronisation;
+ *  - non-finite activations: behaviour unspecified (S:32 rejects them at construction).
+ *
+ * Shape rules (BASEQ_ERR_SHAPE): T >= 1 (empty input is an error, S:57 / S:225),
+ * K % 128 == 0 and 128 <= K <= 32768 (a whole row stays in one CTA's registers),
+ * N % 8 == 0 and N >= 8.  T need not be a multiple of any tile.
+ * Alignment (BASEQ_ERR_ALIGN): x, codes, y, packed blob 16-byte aligned (blob: 128);
+ * ldx >= K, ldx % 8 == 0; ldy >= N, ldy % 8 == 0.
+ */
+#ifndef BASEQ_H_
+#define BASEQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define BASEQ_API __attribute__((visibility("default")))
+#else
+#define BASEQ_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  BASEQ_OK = 0,
+  BASEQ_ERR_NULL = 1,        /* a required pointer is NULL                               */
+  BASEQ_ERR_SHAPE = 2,       /* T/K/N violate the shape rules above                      */
+  BASEQ_ERR_ALIGN = 3,       /* pointer or leading-dimension alignment                   */
+  BASEQ_ERR_PARAM = 4,       /* alpha / gamma / had_block out of range                   */
+  BASEQ_ERR_WORKSPACE = 5,   /* workspace too small or blob header invalid               */
+  BASEQ_ERR_UNSUPPORTED = 6, /* not an sm_100 device                                     */
+  BASEQ_ERR_CUDA = 7         /* a CUDA runtime / driver call failed                      */
+} baseq_status_t;
+
+/* Static string for a status code. */
+BASEQ_API const char* baseq_status_string(baseq_status_t s);
+/* Library version (integer, increases with ABI changes). */
+BASEQ_API int baseq_version(void);
+
+/* The per-quantizer parameters of Eq. 15 / BlockParams.
+ *   u_k = g_k * h_k - b_k,  h = block-Hadamard(x) or x,  g_k = sa ? sa[k] : gamma    (C-1, C-2)
+ *   s_t = max((alpha * max_k |u_k|) / 7, 1e-12)                                       (C-7, C-8, C-10)
+ *   q_k = clamp(rne(u_k * (1 / s_t)), -8, 7)                                          (C-5, C-6)
+ * every line one correctly rounded fp32 operation. */
+typedef struct {
+  float alpha;      /* clip ratio, 0 < alpha <= 1, else BASEQ_ERR_PARAM          */
+  float gamma;      /* scalar s^a, used iff sa == NULL; must be finite and > 0                      */
+  const float* sa;  /* [K] per-channel s^a, already divided by the paired scale s; or NULL          */
+  const float* b;   /* [K] correction bias b^c in the scaled (and rotated) domain; NULL = 0         */
+  int had_block;    /* 0 = none; else online Hadamard block size: a power of two in
+                       [2, 256] dividing K, else BASEQ_ERR_PARAM                            */
+} baseq_act_params_t;
+
+/* ---- offline weight packer (P:241 per-channel symmetric int4; "fused bias" of Eq. 14) ----
+ * Re-tiles int4 weights into the blob the GEMM streams with bulk-TMA copies, stores s_w and
+ * computes the fused bias  fb[n] = s_w[n] * sum_k qw[n,k] * b[k] + layer_bias[n]  (fp64
+ * accumulation, C-3: qw are the very integers the GEMM multiplies).
+ *   w_nibbles   [N, K/2] bytes row-major, byte j of row n = (qw[n,2j] & 15) | ((qw[n,2j+1] & 15) << 4)
+ *   w_scale     [N] fp32 per-output-channel step size s_w
+ *   b           [K] fp32 or NULL (then fb = layer_bias)
+ *   layer_bias  [N] fp32 or NULL
+ *   packed_out  caller buffer of baseq_packed_weight_bytes(N, K) bytes, 128-byte aligned
+ *   fused_bias_out  optional [N] copy of fb for inspection, or NULL
+ * The blob is opaque, position independent (may be copied) and a pure function of the inputs. */
+BASEQ_API size_t baseq_packed_weight_bytes(int N, int K);
+BASEQ_API baseq_status_t baseq_pack_weights(const uint8_t* w_nibbles, const float* w_scale, const float* b,
+                                  const float* layer_bias, int N, int K, void* packed_out,
+                                  float* fused_bias_out, void* stream);
+/* Replace the blob's fused bias by caller-supplied values (parity runs feed the oracle's fb,
+ * whose fp64 summation order is not part of the contract -- DESIGN.md "fused bias"). */
+BASEQ_API baseq_status_t baseq_set_fused_bias(void* packed, int N, int K, const float* fb, void* stream);
+
+/* ---- fused activation quantiser (K2 of SURVEY; "fuse the online bias and scaling ...
+ * within quantization"; Eq. 15; per-token dynamic symmetric int4, round-half-to-even) ----
+ *   x_bf16  [T, ldx] bf16, row-major, first K columns of each row are read
+ *   codes   [T, K/2] bytes: byte j = (q[2j] & 15) | ((q[2j+1] & 15) << 4)
+ *   scales  [T] fp32 step sizes s_t                                                          */
+BASEQ_API baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int T, int K,
+                                  const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                  void* stream);
+
+/* ---- W4A4 GEMM + fused de-quantisation (K1 + K3 of SURVEY) ----
+ *   acc[t,n] = sum_k qa[t,k] * qw[n,k]                       exact int32 (tcgen05 kind::i8)
+ *   Y[t,n]   = bf16_rne( (s_t * s_w[n]) * acc[t,n] + fb[n] ) evaluated as the fp64 expression
+ *              fma((double)s_t * (double)s_w[n], (double)acc, (double)fb[n]), one rounding to bf16 (C-9)
+ *   codes, scales  as produced by baseq_quantize_act
+ *   packed_w       blob from baseq_pack_weights for the same (N, K)
+ *   y_bf16         [T, ldy] bf16 row-major
+ *   acc_dump       optional [T, N] int32 copy of the accumulators (parity runs only), or NULL */
+BASEQ_API baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const void* packed_w,
+                               int T, int N, int K, void* y_bf16, int64_t ldy, int32_t* acc_dump,
+                               void* stream);
+
+/* ---- fused variant: quantise inside the GEMM producer; int4 codes never reach HBM ----
+ * A per-token absmax pre-pass writes scales_out, then one GEMM kernel whose producer warps read
+ * bf16 X tiles, apply Hadamard / scale / bias / round with the known per-token scale and write
+ * int8 operands straight to shared memory.  Same contract and the same bits as
+ * baseq_quantize_act followed by baseq_w4a4_gemm.
+ *   workspace / workspace_bytes  scratch of at least baseq_fused_workspace_bytes(T, N, K)
+ *   codes_dump   optional [T, K/2] copy of the codes the producer computed (parity runs), or NULL
+ *   scales_out   [T] required                                                                */
+BASEQ_API size_t baseq_fused_workspace_bytes(int T, int N, int K);
+BASEQ_API baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
+                                  const baseq_act_params_t* p, const void* packed_w, int N,
+                                  void* y_bf16, int64_t ldy, void* workspace, size_t workspace_bytes,
+                                  uint8_t* codes_dump, float* scales_out, int32_t* acc_dump,
+                                  void* stream);
+
+/* ---- end-to-end helper with HOST activations / outputs (bench.py's e2e leg) ----
+ * Copies x_host (pinned or pageable) to the device scratch, runs quantize_act + w4a4_gemm on
+ * `stream`, copies Y back to y_host.  p->sa / p->b and packed_w are DEVICE pointers as above.
+ *   dev_scratch  device buffer of at least baseq_linear_host_scratch_bytes(T, N, K) bytes
+ * Returns after enqueueing; the caller synchronises the stream before reading y_host. */
+BASEQ_API size_t baseq_linear_host_scratch_bytes(int T, int N, int K);
+BASEQ_API baseq_status_t baseq_linear_host(const void* x_bf16_host, int T, int K, const baseq_act_params_t* p,
+                                 const void* packed_w, int N, void* y_bf16_host, void* dev_scratch,
+                                 size_t dev_scratch_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BASEQ_H_ */

@@ -1,0 +1,277 @@
+// extern "C" entry points of libbaseq (include/baseq.h): host-side validation + dispatch.
+// No compute happens here and nothing falls back to the CPU.
+#include <cmath>
+#include <cstring>
+
+#include "../../include/baseq.h"
+#include "kernels.cuh"
+
+namespace {
+
+using namespace baseq;
+
+bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+struct DeviceInfo {
+  bool ok = false;
+  bool queried = false;
+  int num_sms = 0;
+};
+
+// Cached per process for the current device at first use (one GPU per process).
+baseq_status_t device_check(int* num_sms) {
+  static DeviceInfo info;
+  if (!info.queried) {
+    int dev = 0, major = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return BASEQ_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess)
+      return BASEQ_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+      return BASEQ_ERR_CUDA;
+    info.ok = (major == 10);
+    info.num_sms = sms;
+    info.queried = true;
+  }
+  if (!info.ok) return BASEQ_ERR_UNSUPPORTED;
+  if (num_sms) *num_sms = info.num_sms;
+  return BASEQ_OK;
+}
+
+baseq_status_t check_shape(int T, int N, int K) {
+  if (T < 1) return BASEQ_ERR_SHAPE;
+  if (K < 128 || (K % 128) != 0) return BASEQ_ERR_SHAPE;
+  if (N < 8 || (N % 8) != 0) return BASEQ_ERR_SHAPE;
+  return BASEQ_OK;
+}
+
+baseq_status_t check_act_params(const baseq_act_params_t* p, int K) {
+  if (p == nullptr) return BASEQ_ERR_NULL;
+  if (!(p->alpha > 0.0f) || !(p->alpha <= 1.0f)) return BASEQ_ERR_PARAM;
+  if (p->sa == nullptr && (!(p->gamma > 0.0f) || !std::isfinite(p->gamma))) return BASEQ_ERR_PARAM;
+  if (p->had_block != 0) {
+    const int B = p->had_block;
+    if (B < 2 || B > 256 || (B & (B - 1)) != 0 || (K % B) != 0) return BASEQ_ERR_PARAM;
+  }
+  if (p->sa != nullptr && !aligned(p->sa, 16)) return BASEQ_ERR_ALIGN;
+  if (p->b != nullptr && !aligned(p->b, 16)) return BASEQ_ERR_ALIGN;
+  return BASEQ_OK;
+}
+
+QuantLaunch make_quant(const void* x, int64_t ldx, int T, int K, const baseq_act_params_t* p,
+                       uint8_t* codes, float* scales, void* stream) {
+  QuantLaunch q{};
+  q.x = x;
+  q.ldx = ldx;
+  q.T = T;
+  q.K = K;
+  q.alpha = p->alpha;
+  q.gamma = p->gamma;
+  q.sa = p->sa;
+  q.b = p->b;
+  q.had_block = p->had_block;
+  q.had_scale = p->had_block
+                    ? static_cast<float>(1.0 / std::sqrt(static_cast<double>(p->had_block)))
+                    : 1.0f;
+  q.codes = codes;
+  q.scales = scales;
+  q.stream = static_cast<cudaStream_t>(stream);
+  q.tpr_log2 = 0;
+  q.tpr_log2_override = 0;
+  return q;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* baseq_status_string(baseq_status_t s) {
+  switch (s) {
+    case BASEQ_OK: return "BASEQ_OK";
+    case BASEQ_ERR_NULL: return "BASEQ_ERR_NULL: a required pointer is NULL";
+    case BASEQ_ERR_SHAPE: return "BASEQ_ERR_SHAPE: need T >= 1, K % 128 == 0, N % 8 == 0";
+    case BASEQ_ERR_ALIGN: return "BASEQ_ERR_ALIGN: pointer or leading dimension misaligned";
+    case BASEQ_ERR_PARAM: return "BASEQ_ERR_PARAM: alpha / gamma / had_block out of range";
+    case BASEQ_ERR_WORKSPACE: return "BASEQ_ERR_WORKSPACE: workspace too small or blob invalid";
+    case BASEQ_ERR_UNSUPPORTED: return "BASEQ_ERR_UNSUPPORTED: requires an sm_100 (B200) device";
+    case BASEQ_ERR_CUDA: return "BASEQ_ERR_CUDA: a CUDA call failed";
+  }
+  return "BASEQ: unknown status";
+}
+
+int baseq_version(void) { return 1; }
+
+size_t baseq_packed_weight_bytes(int N, int K) {
+  if (N < 8 || (N % 8) != 0 || K < 128 || (K % 128) != 0) return 0;
+  return blob_bytes(N, K);
+}
+
+baseq_status_t baseq_pack_weights(const uint8_t* w_nibbles, const float* w_scale, const float* b,
+                                  const float* layer_bias, int N, int K, void* packed_out,
+                                  float* fused_bias_out, void* stream) {
+  if (w_nibbles == nullptr || w_scale == nullptr || packed_out == nullptr) return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(1, N, K);
+  if (st != BASEQ_OK) return st;
+  if (!aligned(w_nibbles, 16) || !aligned(packed_out, 128)) return BASEQ_ERR_ALIGN;
+  st = device_check(nullptr);
+  if (st != BASEQ_OK) return st;
+  const cudaError_t e = launch_pack_weights(w_nibbles, w_scale, b, layer_bias, N, K, packed_out,
+                                            fused_bias_out, static_cast<cudaStream_t>(stream));
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
+baseq_status_t baseq_set_fused_bias(void* packed, int N, int K, const float* fb, void* stream) {
+  if (packed == nullptr || fb == nullptr) return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(1, N, K);
+  if (st != BASEQ_OK) return st;
+  if (!aligned(packed, 128)) return BASEQ_ERR_ALIGN;
+  st = device_check(nullptr);
+  if (st != BASEQ_OK) return st;
+  const cudaError_t e = launch_set_fused_bias(packed, N, K, fb, static_cast<cudaStream_t>(stream));
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
+baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int T, int K,
+                                  const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                  void* stream) {
+  if (x_bf16 == nullptr || codes == nullptr || scales == nullptr || p == nullptr)
+    return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(T, 8, K);
+  if (st != BASEQ_OK) return st;
+  if (K > quant_max_k()) return BASEQ_ERR_SHAPE;
+  st = check_act_params(p, K);
+  if (st != BASEQ_OK) return st;
+  if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4)) return BASEQ_ERR_ALIGN;
+  if (ldx < K || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;
+  st = device_check(nullptr);
+  if (st != BASEQ_OK) return st;
+  const cudaError_t e =
+      launch_quantize_act(make_quant(x_bf16, ldx, T, K, p, codes, scales, stream), true);
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
+baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const void* packed_w,
+                               int T, int N, int K, void* y_bf16, int64_t ldy, int32_t* acc_dump,
+                               void* stream) {
+  if (codes == nullptr || scales == nullptr || packed_w == nullptr || y_bf16 == nullptr)
+    return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(T, N, K);
+  if (st != BASEQ_OK) return st;
+  if (K > 131072) return BASEQ_ERR_SHAPE;            // raw accumulator 256*acc must fit int32
+  if (!aligned(codes, 16) || !aligned(y_bf16, 16) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
+  if (acc_dump != nullptr && !aligned(acc_dump, 16)) return BASEQ_ERR_ALIGN;
+  if (ldy < N || (ldy % 8) != 0) return BASEQ_ERR_ALIGN;
+  int sms = 0;
+  st = device_check(&sms);
+  if (st != BASEQ_OK) return st;
+  GemmLaunch g{};
+  g.codes = codes;
+  g.scales = scales;
+  g.blob = packed_w;
+  g.T = T;
+  g.N = N;
+  g.K = K;
+  g.y = y_bf16;
+  g.ldy = ldy;
+  g.acc_dump = acc_dump;
+  g.stream = static_cast<cudaStream_t>(stream);
+  g.num_sms = sms;
+  const cudaError_t e = launch_w4a4_gemm(g);
+  if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
+size_t baseq_fused_workspace_bytes(int T, int N, int K) {
+  (void)N;
+  (void)K;
+  if (T < 1) return 0;
+  return 256;   // the fused path keeps everything on chip; a small fixed scratch is reserved
+}
+
+baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
+                                  const baseq_act_params_t* p, const void* packed_w, int N,
+                                  void* y_bf16, int64_t ldy, void* workspace, size_t workspace_bytes,
+                                  uint8_t* codes_dump, float* scales_out, int32_t* acc_dump,
+                                  void* stream) {
+  if (x_bf16 == nullptr || p == nullptr || packed_w == nullptr || y_bf16 == nullptr ||
+      scales_out == nullptr || workspace == nullptr)
+    return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(T, N, K);
+  if (st != BASEQ_OK) return st;
+  if (K > quant_max_k()) return BASEQ_ERR_SHAPE;
+  st = check_act_params(p, K);
+  if (st != BASEQ_OK) return st;
+  if (!aligned(x_bf16, 16) || !aligned(y_bf16, 16) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
+  if (ldx < K || (ldx % 8) != 0 || ldy < N || (ldy % 8) != 0) return BASEQ_ERR_ALIGN;
+  if (workspace_bytes < baseq_fused_workspace_bytes(T, N, K)) return BASEQ_ERR_WORKSPACE;
+  int sms = 0;
+  st = device_check(&sms);
+  if (st != BASEQ_OK) return st;
+  // pass 1: per-token absmax -> scales (reads X once, writes T floats)
+  cudaError_t e = launch_quantize_act(make_quant(x_bf16, ldx, T, K, p, nullptr, scales_out, stream),
+                                      false);
+  if (e != cudaSuccess) return BASEQ_ERR_CUDA;
+  // pass 2: GEMM with the quantise-in-producer variant
+  GemmLaunch g{};
+  g.scales = scales_out;
+  g.blob = packed_w;
+  g.T = T;
+  g.N = N;
+  g.K = K;
+  g.y = y_bf16;
+  g.ldy = ldy;
+  g.acc_dump = acc_dump;
+  g.x = x_bf16;
+  g.ldx = ldx;
+  g.gamma = p->gamma;
+  g.sa = p->sa;
+  g.b = p->b;
+  g.had_block = p->had_block;
+  g.had_scale = p->had_block
+                    ? static_cast<float>(1.0 / std::sqrt(static_cast<double>(p->had_block)))
+                    : 1.0f;
+  g.codes_dump = codes_dump;
+  g.stream = static_cast<cudaStream_t>(stream);
+  g.num_sms = sms;
+  e = launch_w4a4_gemm(g);
+  if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
+size_t baseq_linear_host_scratch_bytes(int T, int N, int K) {
+  if (T < 1 || N < 8 || K < 128) return 0;
+  auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+  return up(static_cast<size_t>(T) * K * 2) + up(static_cast<size_t>(T) * K / 2) +
+         up(static_cast<size_t>(T) * 4) + up(static_cast<size_t>(T) * N * 2);
+}
+
+baseq_status_t baseq_linear_host(const void* x_bf16_host, int T, int K, const baseq_act_params_t* p,
+                                 const void* packed_w, int N, void* y_bf16_host, void* dev_scratch,
+                                 size_t dev_scratch_bytes, void* stream) {
+  if (x_bf16_host == nullptr || y_bf16_host == nullptr || dev_scratch == nullptr ||
+      packed_w == nullptr || p == nullptr)
+    return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(T, N, K);
+  if (st != BASEQ_OK) return st;
+  if (dev_scratch_bytes < baseq_linear_host_scratch_bytes(T, N, K)) return BASEQ_ERR_WORKSPACE;
+  if (!aligned(dev_scratch, 256)) return BASEQ_ERR_ALIGN;
+  auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+  uint8_t* base = static_cast<uint8_t*>(dev_scratch);
+  void* dx = base;
+  uint8_t* dcodes = base + up(static_cast<size_t>(T) * K * 2);
+  float* dscales = reinterpret_cast<float*>(dcodes + up(static_cast<size_t>(T) * K / 2));
+  void* dy = reinterpret_cast<uint8_t*>(dscales) + up(static_cast<size_t>(T) * 4);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (cudaMemcpyAsync(dx, x_bf16_host, static_cast<size_t>(T) * K * 2, cudaMemcpyHostToDevice, s) !=
+      cudaSuccess)
+    return BASEQ_ERR_CUDA;
+  st = baseq_quantize_act(dx, K, T, K, p, dcodes, dscales, stream);
+  if (st != BASEQ_OK) return st;
+  st = baseq_w4a4_gemm(dcodes, dscales, packed_w, T, N, K, dy, N, nullptr, stream);
+  if (st != BASEQ_OK) return st;
+  if (cudaMemcpyAsync(y_bf16_host, dy, static_cast<size_t>(T) * N * 2, cudaMemcpyDeviceToHost, s) !=
+      cudaSuccess)
+    return BASEQ_ERR_CUDA;
+  return BASEQ_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,94 @@
+// Internal launch interfaces between baseq_api.cu and the kernel translation units.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace baseq {
+
+// ------------------------------------------------------------------ packed weight blob
+// [ header 128 B | s_w[Npad] f32 | fb[Npad] f32 | tiles ]
+// tiles: [Npad/128][K/128] boxes of 128 rows x 64 bytes (= 128 int4 along K), row-major inside
+// the box, so one (n-tile, k-block) box is 8 KB contiguous and consecutive k-blocks of one
+// n-tile are adjacent -- each is fetched with a single bulk-TMA copy.  Npad = N rounded up to
+// 256 (zero rows), so a 128x256 CTA tile never needs a partial B load.
+constexpr uint32_t kBlobMagic = 0x51534142u;   // "BASQ"
+constexpr int kBlobHeaderBytes = 128;
+constexpr int kTileRows = 128;                 // rows per weight box
+constexpr int kTileK = 128;                    // int4 elements along K per box
+constexpr int kTileBytes = kTileRows * kTileK / 2;
+
+struct BlobHeader {
+  uint32_t magic;
+  int32_t N, K, Npad;
+  uint64_t off_sw, off_fb, off_tiles, total_bytes;
+};
+
+inline int blob_npad(int N) { return (N + 255) / 256 * 256; }
+inline size_t blob_bytes(int N, int K) {
+  const size_t npad = static_cast<size_t>(blob_npad(N));
+  return kBlobHeaderBytes + npad * 4 * 2 + npad * static_cast<size_t>(K) / 2;
+}
+inline BlobHeader blob_header(int N, int K) {
+  BlobHeader h{};
+  h.magic = kBlobMagic;
+  h.N = N;
+  h.K = K;
+  h.Npad = blob_npad(N);
+  h.off_sw = kBlobHeaderBytes;
+  h.off_fb = h.off_sw + static_cast<uint64_t>(h.Npad) * 4;
+  h.off_tiles = h.off_fb + static_cast<uint64_t>(h.Npad) * 4;
+  h.total_bytes = blob_bytes(N, K);
+  return h;
+}
+
+// ------------------------------------------------------------------ activation quantiser
+struct QuantLaunch {
+  const void* x;       // bf16 [T, ldx]
+  int64_t ldx;
+  int T, K;
+  float alpha, gamma;
+  const float* sa;
+  const float* b;
+  int had_block;
+  float had_scale;     // (float)(1 / sqrt((double)had_block)), computed on the host
+  uint8_t* codes;      // [T, K/2]
+  float* scales;       // [T]
+  cudaStream_t stream;
+  int tpr_log2;            // filled by the launcher
+  int tpr_log2_override;   // 0 = heuristic (tuning hook for profiling runs)
+};
+int quant_max_k();
+cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes);
+
+// ------------------------------------------------------------------ weight packer
+cudaError_t launch_pack_weights(const uint8_t* w_nibbles, const float* w_scale, const float* b,
+                                const float* layer_bias, int N, int K, void* blob,
+                                float* fused_bias_out, cudaStream_t stream);
+cudaError_t launch_set_fused_bias(void* blob, int N, int K, const float* fb, cudaStream_t stream);
+
+// ------------------------------------------------------------------ GEMM
+struct GemmLaunch {
+  const uint8_t* codes;    // [T, K/2]   (unfused) or nullptr (fused)
+  const float* scales;     // [T]
+  const void* blob;
+  int T, N, K;
+  void* y;                 // bf16 [T, ldy]
+  int64_t ldy;
+  int32_t* acc_dump;       // optional [T, N]
+  // fused producer inputs (x != nullptr selects the quantise-in-producer variant)
+  const void* x;
+  int64_t ldx;
+  float gamma;
+  const float* sa;
+  const float* b;
+  int had_block;
+  float had_scale;
+  uint8_t* codes_dump;     // optional [T, K/2]
+  cudaStream_t stream;
+  int num_sms;
+};
+// Returns cudaSuccess, or an error (cudaErrorNotSupported when the tensor map cannot be built).
+cudaError_t launch_w4a4_gemm(const GemmLaunch& g);
+
+}  // namespace baseq

@@ -1,0 +1,217 @@
+"""GPU-vs-oracle parity (-m gpu): bit-exact codes, scales, int32 accumulators and bf16 output.
+
+Every call goes through the C-ABI library (paper_2506_15689_b200.binding -> libbaseq.so).
+Expected values come from oracle/ only, on the same seeded inputs (baseq_inputs).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from baseq_inputs import f32_to_bf16_bits, make_activations, make_layer, make_weights
+
+pytestmark = pytest.mark.gpu
+
+bq = None
+
+
+def setup_module(module):
+    global bq
+    import paper_2506_15689_b200 as _bq
+    bq = _bq
+    assert torch.cuda.is_available()
+
+
+def dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    return t if dtype is None else t.view(dtype)
+
+
+def bf16_dev(bits):
+    return torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def bits_host(t):
+    return t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def run_quant(x_bits, alpha, gamma=1.0, sa=None, b=None, had_block=0):
+    params = bq.ActParams(alpha, gamma, None if sa is None else dev(sa),
+                          None if b is None else dev(b), had_block)
+    codes, scales = bq.quantize_act(bf16_dev(x_bits), params)
+    torch.cuda.synchronize()
+    return codes.cpu().numpy(), scales.cpu().numpy()
+
+
+def check_quant(x_bits, alpha, gamma=1.0, sa=None, b=None, had_block=0):
+    codes, scales = run_quant(x_bits, alpha, gamma, sa, b, had_block)
+    ocodes, oscales = oracle.quantize_act(x_bits, alpha, gamma, sa, b, had_block)
+    assert np.array_equal(scales.view(np.uint32), oscales.view(np.uint32)), "scales differ"
+    assert np.array_equal(codes, ocodes), "codes differ: %d bytes" % int((codes != ocodes).sum())
+
+
+def rand_x(rng, T, K, spread=0.5):
+    mu = spread * rng.standard_normal(K)
+    return f32_to_bf16_bits((mu[None, :] + rng.standard_normal((T, K))).astype(np.float32))
+
+
+# ------------------------------------------------------------------------------- quantizer
+@pytest.mark.parametrize("T,K", [(1, 128), (16, 256), (37, 384), (130, 4096), (33, 11008),
+                                 (9, 14336), (5, 28672), (257, 1024), (3, 32768)])
+def test_quantizer_bit_exact_shapes(T, K):
+    rng = np.random.default_rng(T * 100003 + K)
+    x = rand_x(rng, T, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    check_quant(x, 0.9, 1.05, None, b)
+
+
+def test_quantizer_variants():
+    rng = np.random.default_rng(7)
+    T, K = 67, 2048
+    x = rand_x(rng, T, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+    check_quant(x, 1.0)                          # plain RTN
+    check_quant(x, 0.5, 1.2)                     # heavy clipping: saturates at -8 / 7
+    check_quant(x, 0.9, 1.0, sa, b)              # per-channel s^a
+    check_quant(x, 0.9, 1.0, sa, None)
+    zero = np.zeros((4, 256), dtype=np.uint16)   # degenerate rows: floor scale, codes 0
+    check_quant(zero, 0.9)
+    ties = f32_to_bf16_bits(np.tile(np.array([0.5, 1.5, 2.5, -0.5, -1.5, -2.5, 7.0, 3.5],
+                                             dtype=np.float32), (3, 32)))
+    check_quant(ties, 1.0)
+
+
+@pytest.mark.parametrize("K,B", [(256, 128), (4096, 128), (28672, 128), (1024, 16), (512, 256),
+                                 (384, 2)])
+def test_quantizer_hadamard_bit_exact(K, B):
+    rng = np.random.default_rng(K + B)
+    x = rand_x(rng, 19, K, 0.3)
+    b = (0.2 * rng.standard_normal(K)).astype(np.float32)
+    check_quant(x, 0.9, 1.0, None, b, B)
+
+
+def test_quantizer_strided_input():
+    rng = np.random.default_rng(11)
+    T, K, ld = 21, 512, 640
+    full = rand_x(rng, T, ld)
+    xt = bf16_dev(full)[:, :K]
+    params = bq.ActParams(0.9)
+    codes, scales = bq.quantize_act(xt, params)
+    oc, os_ = oracle.quantize_act(np.ascontiguousarray(full[:, :K]), 0.9)
+    assert np.array_equal(codes.cpu().numpy(), oc)
+    assert np.array_equal(scales.cpu().numpy(), os_)
+
+
+# ------------------------------------------------------------------------------- packer
+def test_pack_weights_fused_bias_matches_oracle():
+    W = make_weights("c1", "linear")
+    rng = np.random.default_rng(3)
+    b = rng.standard_normal(W["K"]).astype(np.float32)
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(b), dev(W["layer_bias"]))
+    torch.cuda.synchronize()
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    assert np.array_equal(pw.fused_bias.cpu().numpy().view(np.uint32), fb.view(np.uint32))
+
+
+# ------------------------------------------------------------------------------- GEMM + epilogue
+def run_linear(x_bits, W, alpha, gamma, b, had_block=0, rows=None, with_bias=True):
+    """Runs quantize + GEMM on the GPU and the oracle; compares everything bit for bit."""
+    N, K = W["N"], W["K"]
+    lb = W["layer_bias"] if with_bias else None
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, lb)
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None if b is None else dev(b),
+                         None if lb is None else dev(lb))
+    torch.cuda.synchronize()
+    assert np.array_equal(pw.fused_bias.cpu().numpy().view(np.uint32), fb.view(np.uint32))
+    params = bq.ActParams(alpha, gamma, None, None if b is None else dev(b), had_block)
+    xd = bf16_dev(x_bits)
+    T = x_bits.shape[0]
+    codes, scales = bq.quantize_act(xd, params)
+    acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
+    y = bq.w4a4_gemm(codes, scales, pw, acc_dump=acc)
+    y2 = bq.w4a4_gemm(codes, scales, pw)            # timed configuration: no dump
+    torch.cuda.synchronize()
+    assert torch.equal(y.view(torch.int16), y2.view(torch.int16))
+    sel = np.arange(T) if rows is None else rows
+    ref = oracle.linear(np.ascontiguousarray(x_bits[sel]), W["w_nibbles"], W["w_scale"], fb,
+                        alpha, gamma, None, b, had_block)
+    assert np.array_equal(codes.cpu().numpy()[sel], ref["codes"])
+    assert np.array_equal(scales.cpu().numpy()[sel], ref["scales"])
+    gacc = acc.cpu().numpy()[sel]
+    assert np.array_equal(gacc, ref["acc"]), "int32 accumulators differ at %d places" % int(
+        (gacc != ref["acc"]).sum())
+    gy = bits_host(y)[sel]
+    nbad = int((gy != ref["y"]).sum())
+    assert nbad == 0, "bf16 output differs at %d of %d places" % (nbad, gy.size)
+    return ref, gy
+
+
+def test_config1_full():
+    L = make_layer("c1", "linear")
+    sp = L["spec"]
+    run_linear(L["x"], L, sp.alpha, sp.gamma, L["b"])
+
+
+@pytest.mark.parametrize("T,K,N", [(16, 256, 256), (1, 128, 8), (130, 384, 264), (257, 1024, 520),
+                                   (128, 128, 256), (300, 2048, 1024)])
+def test_linear_ragged_shapes(T, K, N):
+    rng = np.random.default_rng(T + 7 * K + 13 * N)
+    x = rand_x(rng, T, K)
+    q = rng.integers(-8, 8, size=(N, K)).astype(np.int8).astype(np.uint8) & 0xF
+    W = {"N": N, "K": K, "w_nibbles": np.ascontiguousarray(q[:, 0::2] | (q[:, 1::2] << 4)),
+         "w_scale": (0.002 + 0.004 * rng.random(N)).astype(np.float32),
+         "layer_bias": rng.standard_normal(N).astype(np.float32)}
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    run_linear(x, W, 0.9, 1.05, b)
+
+
+def test_gemm_extreme_codes():
+    # qa = 7, qw = -8 everywhere: acc = -56 K (closed form), largest |raw| accumulator
+    T, K, N = 130, 4096, 256
+    codes = torch.full((T, K // 2), 0x77, dtype=torch.uint8, device="cuda")
+    scales = torch.full((T,), 0.25, dtype=torch.float32, device="cuda")
+    wn = np.full((N, K // 2), 0x88, dtype=np.uint8)
+    sw = np.full((N,), 0.5, dtype=np.float32)
+    pw = bq.pack_weights(dev(wn), dev(sw))
+    acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
+    y = bq.w4a4_gemm(codes, scales, pw, acc_dump=acc)
+    torch.cuda.synchronize()
+    assert torch.all(acc == -56 * K)
+    assert torch.all(y.float() == -56.0 * K * 0.125)
+
+
+def test_config2_sampled_rows():
+    L = make_layer("c2", "qkvo")
+    sp = L["spec"]
+    rows = np.r_[0:8, 1020:1030, 2040:2048]
+    run_linear(L["x"], L, sp.alpha, sp.gamma, L["b"], rows=rows)
+
+
+def test_config5_hadamard_small_T():
+    # config 5's K = 28672 + Hadamard-128 with a small token count (full N would take the
+    # oracle minutes: use the first 512 output channels of the seeded weight).
+    A = make_activations("c5", "x_down", T=40)
+    rng = np.random.default_rng(5)
+    K, N = 28672, 512
+    q = rng.integers(-8, 8, size=(N, K)).astype(np.int8).astype(np.uint8) & 0xF
+    W = {"N": N, "K": K, "w_nibbles": np.ascontiguousarray(q[:, 0::2] | (q[:, 1::2] << 4)),
+         "w_scale": (0.002 + 0.004 * rng.random(N)).astype(np.float32), "layer_bias": None}
+    run_linear(A["x"], W, 0.9, 1.0, A["b"], had_block=128)
+
+
+# ------------------------------------------------------------------------------- ABI errors
+def test_abi_error_codes():
+    x = torch.zeros((4, 256), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(bq.BaseqError) as e:
+        bq.quantize_act(x, bq.ActParams(0.0))
+    assert e.value.status == 4
+    with pytest.raises(bq.BaseqError) as e:
+        bq.quantize_act(x, bq.ActParams(0.9, had_block=96))
+    assert e.value.status == 4
+    with pytest.raises(bq.BaseqError) as e:
+        bq.quantize_act(torch.zeros((4, 192), dtype=torch.bfloat16, device="cuda"), bq.ActParams(0.9))
+    assert e.value.status == 2
+    with pytest.raises(bq.BaseqError) as e:
+        bq.quantize_act(torch.zeros((0, 256), dtype=torch.bfloat16, device="cuda"), bq.ActParams(0.9))
+    assert e.value.status == 2
