@@ -1,0 +1,393 @@
+"""bench.py -- headline benchmark of the BASE-Q W4A4 linear hot path on B200.
+
+One "step" = one pass of the whole hot path over the Llama-2-7B MLP pair of BASELINE.json
+configs[2] (T = 4096 tokens): quantise x_mlp once -> up GEMM -> gate GEMM -> quantise x_down ->
+down GEMM (5 kernel launches, all through libbaseq's C ABI).  This is the 4096-token prefill
+shape `north_star` quotes its targets on.  Inputs are seeded synthetic tensors (baseq_inputs).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config c3]
+
+Prints ONE JSON line.  With --impl reference the oracle (CPU,
+as it stands) is timed on a bounded token sample of the same workload.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from baseq_inputs import CONFIGS, make_activations, make_weights  # noqa: E402
+
+METRIC = "fused W4A4 linear tokens/s"
+UNIT = "tokens/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return {"hbm_gbs": p["hbm_gbs"], "bf16_burst": p["bf16_tflops"],
+                "bf16_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]),
+                "source": "measured"}
+    # fallback stated in /opt/skills/guides/B200_PROFILING.md
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+def step_plan(config):
+    """Groups the config's layers by the activation they share: [(act, [layer specs])]."""
+    plan, seen = [], {}
+    for sp in CONFIGS[config]:
+        if sp.act not in seen:
+            seen[sp.act] = len(plan)
+            plan.append((sp.act, []))
+        plan[seen[sp.act]][1].append(sp)
+    return plan
+
+
+def dist_info():
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), ws
+
+
+def max_over_ranks(value, world_size, device=None):
+    """MAX over ranks of a python float (torch.distributed; works with nccl and gloo)."""
+    if world_size == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            pass
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop_evt.wait(0.005)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------ oracle legs
+def oracle_step(config, data, n_tokens):
+    """One pass of the hot path on the first n_tokens tokens with the CPU oracle (as it stands)."""
+    import oracle
+    for act, specs in step_plan(config):
+        A = data["acts"][act]
+        sp0 = specs[0]
+        x = np.ascontiguousarray(A["x"][:n_tokens])
+        codes, scales = oracle.quantize_act(x, sp0.alpha, sp0.gamma, None, A["b"], sp0.had_block)
+        for sp in specs:
+            W = data["weights"][sp.name]
+            acc = oracle.gemm_i32(codes, W["w_nibbles"])
+            oracle.epilogue(acc, scales, W["w_scale"], W["fb_oracle"])
+
+
+def prepare_oracle_fb(config, data):
+    import oracle
+    for act, specs in step_plan(config):
+        for sp in specs:
+            W = data["weights"][sp.name]
+            if "fb_oracle" not in W:
+                W["fb_oracle"] = oracle.fused_bias(W["w_nibbles"], W["w_scale"],
+                                                   data["acts"][act]["b"], W["layer_bias"])
+
+
+def gen_data(config, rank):
+    acts, weights = {}, {}
+    for act, specs in step_plan(config):
+        acts[act] = make_activations(config, act)
+        for sp in specs:
+            weights[sp.name] = make_weights(config, sp.name)
+    return {"acts": acts, "weights": weights}
+
+
+def macs_per_token(config):
+    return sum(sp.K * sp.N for sp in CONFIGS[config])
+
+
+def run_reference(args):
+    rank, _, ws = dist_info()
+    if rank != 0:
+        return
+    config = args.config
+    data = gen_data(config, 0)
+    prepare_oracle_fb(config, data)
+    # bounded sample: tokens per step sized for ~1.5 s of single-core work at ~1.2 GMAC/s
+    n_tok = max(1, min(CONFIGS[config][0].T, int(1.8e9 / macs_per_token(config))))
+    for _ in range(min(args.warmup, 1)):
+        oracle_step(config, data, n_tok)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(config, data, n_tok)
+    dt = time.perf_counter() - t0
+    value = n_tok * args.steps / dt
+    sample = "first %d tokens of each activation per step, all layers, full N and K" % n_tok
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int4xint4->int32; fp32 quantizer; fp64 epilogue",
+            "data": "synthetic", "config": workload_config(config),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(config):
+    layers = ["%s %dx%dx%d" % (sp.name, sp.T, sp.K, sp.N) for sp in CONFIGS[config]]
+    return {"workload": "BASELINE.json configs[%d] (%s): %s; one step = quantise each shared "
+                        "activation once + one W4A4 GEMM per layer" % (int(config[1]) - 1, config, "; ".join(layers)),
+            "tokens_per_step": CONFIGS[config][0].T,
+            "l2": "per-step footprint (activations + packed weights + outputs) exceeds the 126 MB L2; no explicit flush"}
+
+
+# ------------------------------------------------------------------------------ GPU arm
+def run_gpu(args):
+    import torch
+    import paper_2506_15689_b200 as bq
+
+    rank, local_rank, ws = dist_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if ws > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    config = args.config
+    peaks = load_peaks()
+    data = gen_data(config, rank)
+    plan = step_plan(config)
+    T = CONFIGS[config][0].T
+
+    def dev(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    acts, layers = {}, {}
+    for act, specs in plan:
+        A = data["acts"][act]
+        sp0 = specs[0]
+        xb = torch.from_numpy(A["x"].view(np.int16)).cuda().view(torch.bfloat16)
+        bdev = dev(A["b"])
+        acts[act] = {"x": xb, "params": bq.ActParams(sp0.alpha, sp0.gamma, None, bdev, sp0.had_block),
+                     "codes": torch.empty((T, sp0.K // 2), dtype=torch.uint8, device="cuda"),
+                     "scales": torch.empty((T,), dtype=torch.float32, device="cuda"), "K": sp0.K}
+        for sp in specs:
+            W = data["weights"][sp.name]
+            pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), bdev,
+                                 None if W["layer_bias"] is None else dev(W["layer_bias"]))
+            layers[sp.name] = {"pw": pw, "y": torch.empty((T, sp.N), dtype=torch.bfloat16, device="cuda"),
+                               "spec": sp}
+    torch.cuda.synchronize()
+
+    kernels = []   # (kind, name, algorithmic work) in launch order
+    for act, specs in plan:
+        kernels.append(("quant", act, 2.5 * T * acts[act]["K"]))
+        for sp in specs:
+            kernels.append(("gemm", sp.name, 2.0 * T * sp.N * sp.K))
+
+    def step(events=None):
+        i = 0
+        for act, specs in plan:
+            a = acts[act]
+            bq.quantize_act(a["x"], a["params"], a["codes"], a["scales"])
+            if events is not None:
+                i += 1
+                events[i].record()
+            for sp in specs:
+                L = layers[sp.name]
+                bq.w4a4_gemm(a["codes"], a["scales"], L["pw"], L["y"])
+                if events is not None:
+                    i += 1
+                    events[i].record()
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if ws > 1:
+        dist.barrier()
+    nk = len(kernels)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(nk + 1)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        evs[k][0].record()
+        step(evs[k])
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    if ws > 1:
+        dist.barrier()
+    total_ms = evs[0][0].elapsed_time(evs[-1][nk])
+    total_ms = max_over_ranks(total_ms, ws, torch.device("cuda", local_rank))
+    per_kernel = np.zeros(nk)
+    for k in range(args.steps):
+        for i in range(nk):
+            per_kernel[i] += evs[k][i].elapsed_time(evs[k][i + 1])
+    per_kernel /= args.steps
+    ms_per_step = total_ms / args.steps
+    value = ws * T * args.steps / (total_ms * 1e-3)
+
+    gemm_ms = sum(per_kernel[i] for i, kd in enumerate(kernels) if kd[0] == "gemm")
+    gemm_ops = sum(kd[2] for kd in kernels if kd[0] == "gemm")
+    n_gemm = sum(1 for kd in kernels if kd[0] == "gemm")
+    quant_ms = sum(per_kernel[i] for i, kd in enumerate(kernels) if kd[0] == "quant")
+    quant_bytes = sum(kd[2] for kd in kernels if kd[0] == "quant")
+    tops = gemm_ops / (gemm_ms * 1e-3) / 1e12
+    int8_peak = 2.0 * peaks["bf16_sustained"]
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("w4a4_gemm_kernel_bytes_per_launch")
+    roofline = {"bound": "tensor", "kernel": "w4a4_gemm_kernel", "achieved": tops, "peak": int8_peak,
+                "unit": "TFLOP/s", "frac": tops / int8_peak, "traffic": traffic,
+                "peak_source": "2 x %s bf16 sustained (%s MEASURED_PEAKS.json; int8:bf16 nominal ratio 2)"
+                               % (peaks["bf16_sustained"], peaks["source"]),
+                "frac_of_nominal_4500": tops / 4500.0,
+                "avg_launch_ms": gemm_ms / n_gemm, "share_of_step": gemm_ms / per_kernel.sum()}
+    qgbs = quant_bytes / (quant_ms * 1e-3) / 1e9
+    roofline_q = {"bound": "hbm", "kernel": "quantize_act_kernel", "achieved": qgbs,
+                  "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": qgbs / peaks["hbm_gbs"],
+                  "frac_of_nominal_8000": qgbs / 8000.0, "share_of_step": quant_ms / per_kernel.sum()}
+    per_layer = [{"kernel": kd[0], "name": kd[1], "ms": float(per_kernel[i]),
+                  "rate": float(kd[2] / (per_kernel[i] * 1e-3) / (1e12 if kd[0] == "gemm" else 1e9)),
+                  "rate_unit": "TOP/s" if kd[0] == "gemm" else "GB/s"} for i, kd in enumerate(kernels)]
+
+    # ---- end-to-end: HOST buffers through baseq_linear_host (H2D of X and D2H of Y timed)
+    e2e = run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "int4xint4->int32 (tcgen05 kind::i8); fp32 quantizer; bf16 out",
+            "data": "synthetic", "config": workload_config(config), "clocks": clocks,
+            "e2e": e2e, "gpu_launches": nk * args.steps, "roofline": roofline,
+            "roofline_quantizer": roofline_q, "kernels": per_layer}
+    if rank == 0 and ws == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(config, data, plan, layers, torch)
+    if rank == 0:
+        print(json.dumps(line))
+    if ws > 1:
+        dist.destroy_process_group()
+
+
+def run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank):
+    from paper_2506_15689_b200.binding import linear_host_scratch_bytes
+    host_x, host_y, h2d, d2h, scratch_bytes = {}, {}, 0, 0, 0
+    for act, specs in plan:
+        host_x[act] = torch.from_numpy(data["acts"][act]["x"].view(np.int16)).view(torch.bfloat16).pin_memory()
+        for sp in specs:
+            host_y[sp.name] = torch.empty((T, sp.N), dtype=torch.bfloat16).pin_memory()
+            h2d += T * sp.K * 2
+            d2h += T * sp.N * 2
+            scratch_bytes = max(scratch_bytes, linear_host_scratch_bytes(T, sp.N, sp.K))
+    scratch = torch.empty(scratch_bytes, dtype=torch.uint8, device="cuda")
+
+    def step():
+        for act, specs in plan:
+            for sp in specs:
+                bq.linear_host(host_x[act], acts[act]["params"], layers[sp.name]["pw"],
+                               host_y[sp.name], scratch)
+
+    for _ in range(min(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    steps = max(3, min(args.steps, 10))
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = max_over_ranks(e0.elapsed_time(e1), ws, torch.device("cuda", local_rank))
+    # the result read back must be the kernels' output
+    name = plan[0][1][0].name
+    same = bool(torch.equal(host_y[name].view(torch.int16), layers[name]["y"].cpu().view(torch.int16)))
+    return {"value": ws * T * steps / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "steps": steps, "ms_per_step": ms / steps,
+            "api": "baseq_linear_host per layer (pinned host X in, pinned host Y out)",
+            "matches_device_path": same}
+
+
+def cpu_baseline(config, data, plan, layers, torch):
+    """Oracle as it stands, one core, on the first n tokens; also spot-checks GPU parity."""
+    prepare_oracle_fb(config, data)
+    n_tok = max(1, min(CONFIGS[config][0].T, int(45e9 / macs_per_token(config))))
+    t0 = time.perf_counter()
+    oracle_step(config, data, n_tok)
+    dt = time.perf_counter() - t0
+    import oracle
+    ok = True
+    for act, specs in plan:
+        A = data["acts"][act]
+        sp = specs[0]
+        W = data["weights"][sp.name]
+        ref = oracle.linear(np.ascontiguousarray(A["x"][:4]), W["w_nibbles"], W["w_scale"],
+                            W["fb_oracle"], sp.alpha, sp.gamma, None, A["b"], sp.had_block)
+        got = layers[sp.name]["y"][:4].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        ok = ok and bool(np.array_equal(got, ref["y"]))
+    return {"value": n_tok / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "first %d of %d tokens, all layers, full N and K, %.1f s" % (
+                n_tok, CONFIGS[config][0].T, dt),
+            "gpu_bit_exact_on_4_tokens": ok}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="baseq", choices=["baseq", "reference"])
+    ap.add_argument("--config", default="c3", choices=sorted(CONFIGS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -133,10 +133,10 @@ baseq_status_t baseq_set_fused_bias(void* packed, int N, int K, const float* fb,
 baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int T, int K,
                                   const baseq_act_params_t* p, uint8_t* codes, float* scales,
                                   void* stream) {
+  baseq_status_t st = check_shape(T, 8, K);     // empty input is a shape error
+  if (st != BASEQ_OK) return st;
   if (x_bf16 == nullptr || codes == nullptr || scales == nullptr || p == nullptr)
     return BASEQ_ERR_NULL;
-  baseq_status_t st = check_shape(T, 8, K);
-  if (st != BASEQ_OK) return st;
   if (K > quant_max_k()) return BASEQ_ERR_SHAPE;
   st = check_act_params(p, K);
   if (st != BASEQ_OK) return st;
