@@ -1,6 +1,7 @@
 // extern "C" entry points of libbaseq (include/baseq.h): host-side validation + dispatch.
 // No compute happens here and nothing falls back to the CPU.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "../../include/baseq.h"
@@ -78,6 +79,16 @@ QuantLaunch make_quant(const void* x, int64_t ldx, int T, int K, const baseq_act
   q.tpr_log2 = 0;
   q.tpr_log2_override = 0;
   return q;
+}
+
+// Tuning hook for profiling runs only: BASEQ_GEMM_CTA_GROUP=1 selects the single-CTA tiles.
+int gemm_cta_group() {
+  static int v = 0;
+  if (v == 0) {
+    const char* e = std::getenv("BASEQ_GEMM_CTA_GROUP");
+    v = (e != nullptr && e[0] == '1') ? 1 : 2;
+  }
+  return v;
 }
 
 }  // namespace
@@ -175,6 +186,7 @@ baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const 
   g.acc_dump = acc_dump;
   g.stream = static_cast<cudaStream_t>(stream);
   g.num_sms = sms;
+  g.cta_group = gemm_cta_group();
   const cudaError_t e = launch_w4a4_gemm(g);
   if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
@@ -232,6 +244,7 @@ baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
   g.codes_dump = codes_dump;
   g.stream = static_cast<cudaStream_t>(stream);
   g.num_sms = sms;
+  g.cta_group = gemm_cta_group();
   e = launch_w4a4_gemm(g);
   if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;

@@ -7,14 +7,16 @@
 namespace baseq {
 
 // ------------------------------------------------------------------ packed weight blob
-// [ header 128 B | s_w[Npad] f32 | fb[Npad] f32 | tiles ]
-// tiles: [Npad/128][K/128] boxes of 128 rows x 64 bytes (= 128 int4 along K), row-major inside
-// the box, so one (n-tile, k-block) box is 8 KB contiguous and consecutive k-blocks of one
-// n-tile are adjacent -- each is fetched with a single bulk-TMA copy.  Npad = N rounded up to
-// 256 (zero rows), so a 128x256 CTA tile never needs a partial B load.
+// [ header 128 B | s_w[Npad] f32 | fb[Npad] f32 | boxes ]
+// boxes: [Npad/kTileRows][K/128] boxes of kTileRows rows x 64 bytes (= 128 int4 along K),
+// row-major inside the box, so one (row group, k-block) box is contiguous and consecutive
+// k-blocks of one row group are adjacent -- each is fetched with a single bulk-TMA copy.
+// kTileRows = half a GEMM tile's N extent: each CTA of a CTA pair streams one row group.
+// Npad = N rounded up to the tile's N extent (zero rows), so no partial B load exists.
 constexpr uint32_t kBlobMagic = 0x51534142u;   // "BASQ"
 constexpr int kBlobHeaderBytes = 128;
-constexpr int kTileRows = 128;                 // rows per weight box
+constexpr int kGemmBN = 192;                   // output channels per GEMM tile (UMMA N)
+constexpr int kTileRows = kGemmBN / 2;         // rows per weight box
 constexpr int kTileK = 128;                    // int4 elements along K per box
 constexpr int kTileBytes = kTileRows * kTileK / 2;
 
@@ -24,7 +26,7 @@ struct BlobHeader {
   uint64_t off_sw, off_fb, off_tiles, total_bytes;
 };
 
-inline int blob_npad(int N) { return (N + 255) / 256 * 256; }
+inline int blob_npad(int N) { return (N + kGemmBN - 1) / kGemmBN * kGemmBN; }
 inline size_t blob_bytes(int N, int K) {
   const size_t npad = static_cast<size_t>(blob_npad(N));
   return kBlobHeaderBytes + npad * 4 * 2 + npad * static_cast<size_t>(K) / 2;
@@ -87,6 +89,7 @@ struct GemmLaunch {
   uint8_t* codes_dump;     // optional [T, K/2]
   cudaStream_t stream;
   int num_sms;
+  int cta_group;           // 2 = CTA pairs (default), 1 = single CTA per tile (tuning hook)
 };
 // Returns cudaSuccess, or an error (cudaErrorNotSupported when the tensor map cannot be built).
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g);

@@ -2,15 +2,25 @@
 // PAPER.md:307).  sm_100a has no int4 MMA kind, so int4 nibbles are expanded on-chip to int8
 // and multiplied with tcgen05.mma kind::i8 (exact int32 accumulation in TMEM).
 //
-// Persistent, warp-specialised, one CTA per SM, 128x256 output tile, K-block = 128:
-//   warp 0      producer  : TMA (2-D tensor map for A codes, 1-D bulk copies for the packed
-//                           weight boxes) into a ring of PACKED stages
-//   warps 8-15  unpackers : packed int4 -> int8 (x16 trick, below) into a ring of UNPACKED
-//                           stages in the SWIZZLE_128B K-major layout the MMA reads
-//   warp 1      MMA       : one elected thread issues 4 x tcgen05.mma (K = 32 each) per K-block
-//                           into one of two 256-column TMEM accumulators
-//   warps 4-7   epilogue  : tcgen05.ld -> dequant (+ fused bias) -> bf16 -> global; overlaps the
-//                           next tile's main loop through the second TMEM accumulator
+// The r1a kernel staged both operands packed -> smem -> unpack -> smem -> MMA and ran exactly at
+// the shared-memory bandwidth limit (144 KB of smem traffic per 128x256x128 k-block against a
+// 64 KB budget at the int8 MMA rate; profiles/r1a.md).  This version removes most of it:
+//   * the activation operand A never touches shared memory: four warps (thread = token row) load
+//     64 B of packed codes per k-block straight from global/L2 into registers, expand them and
+//     write int8 to TENSOR MEMORY with tcgen05.st; the MMA takes A from TMEM (.ts form);
+//   * a CTA PAIR (cta_group::2, M = 256) shares the weight operand: each CTA stages and
+//     expands only half of the tile's N rows.
+// Per CTA and k-block the shared-memory traffic is  BN/2 x (64 B TMA write + 64 B unpack read +
+// 128 B unpack write + 128 B MMA read) = 36 KB at BN = 192  against 48 KB of budget.
+//
+// Persistent, warp-specialised, one CTA per SM, 512 threads:
+//   warp 0      B producer: one bulk-TMA copy per k-block of this CTA's weight box (packed ring)
+//   warp 1      MMA issuer (leader CTA of the pair only): 4 x tcgen05.mma.kind::i8 (K = 32) per
+//               k-block into one of two BN-column TMEM accumulators; commits multicast to both CTAs
+//   warps 4-7   epilogue: tcgen05.ld -> dequant (+ fused bias) -> bf16 -> global; overlaps the
+//               next tile's main loop through the second accumulator
+//   warps 8-11  A loaders (or, in the fused variant, the quantise-in-producer warps)
+//   warps 12-15 B unpackers: packed int4 -> int8 into SWIZZLE_128B K-major stages
 //
 // x16 unpack: for a 32-bit word w holding 8 two's-complement nibbles,
 //   lo = (w << 4) & 0xF0F0F0F0   -> 4 signed bytes = 16 * (even-k codes)
@@ -26,41 +36,49 @@
 namespace baseq {
 namespace {
 
-constexpr int BM = 128;                 // tokens per tile (UMMA M)
-constexpr int BN = 256;                 // output channels per tile (UMMA N)
+constexpr int BM = 128;                 // token rows per CTA (TMEM lanes)
+constexpr int BN = kGemmBN;             // output channels per tile (UMMA N)
 constexpr int BK = 128;                 // int4 elements along K per stage
-constexpr int kPackedA = BM * BK / 2;   // 8 KB
-constexpr int kPackedB = BN * BK / 2;   // 16 KB
-constexpr int kPackedStage = kPackedA + kPackedB;
-constexpr int kUnpackedA = BM * BK;     // 16 KB (int8)
-constexpr int kUnpackedB = BN * BK;     // 32 KB
-constexpr int kUnpackedStage = kUnpackedA + kUnpackedB;
-constexpr int kPStages = 3;
-constexpr int kUStages = 3;
+constexpr int kStages = 4;              // operand stages: A in TMEM (32 columns), B unpacked in smem
+constexpr int kPStages = 4;             // packed-B ring
 constexpr int kAccStages = 2;
+constexpr int kACol0 = kAccStages * BN; // first TMEM column of the A stages
 constexpr int kTmemCols = 512;
+constexpr int kPackedA = BM * BK / 2;    // 8 KB of packed codes per CTA and k-block
+static_assert(kACol0 + kStages * (BK / 4) <= kTmemCols, "TMEM budget");
+static_assert(BN % 32 == 0 && BN <= 256, "UMMA N");
 
 constexpr int kNumThreads = 512;
 constexpr int kProducerWarp = 0;
 constexpr int kMmaWarp = 1;
-constexpr int kEpiWarp0 = 4;            // warps 4..7  (warp % 4 = TMEM lane quarter)
-constexpr int kUnpackWarp0 = 8;         // warps 8..15
-constexpr int kNumUnpackWarps = 8;
+constexpr int kEpiWarp0 = 4;            // warps 4..7   (warp % 4 = TMEM lane quarter)
+constexpr int kAWarp0 = 8;              // warps 8..11  (warp % 4 = TMEM lane quarter)
+constexpr int kUnpackWarp0 = 12;        // warps 12..15
+constexpr int kNumUnpackWarps = 4;
 
-struct __align__(8) Barriers {
-  uint64_t pfull[kPStages], pempty[kPStages];
-  uint64_t ufull[kUStages], uempty[kUStages];
-  uint64_t tfull[kAccStages], tempty[kAccStages];
-  uint32_t tmem_base;
+template <int CG>
+struct Cfg {
+  static constexpr int kBRows = BN / CG;                   // weight rows staged per CTA
+  static constexpr int kPackedB = kBRows * BK / 2;
+  static constexpr int kPackedStage = kPackedA + kPackedB;  // multiple of 1024 (swizzle alignment)
+  static constexpr int kUnpackedStage = kBRows * BK;
+  static constexpr int kFullCount = CG * (4 + kNumUnpackWarps);
+  static constexpr int kTemptyCount = CG * 4;
+  static constexpr int kSmemBytes = 1024 + kStages * kUnpackedStage + kPStages * kPackedStage + 256;
 };
 
-constexpr int kSmemBytes = 1024 /*align slack*/ + kUStages * kUnpackedStage +
-                           kPStages * kPackedStage + 256 /*barriers*/;
+struct __align__(8) Barriers {
+  uint64_t pfull[kPStages], pempty[kPStages];   // packed-B ring, CTA-local
+  uint64_t full[kStages];                       // operand stage ready   (waited on in the leader CTA)
+  uint64_t empty[kStages];                      // operand stage free    (every CTA; MMA commit)
+  uint64_t tfull[kAccStages];                   // accumulator ready     (every CTA; MMA commit)
+  uint64_t tempty[kAccStages];                  // accumulator drained   (waited on in the leader CTA)
+  uint32_t tmem_base;
+};
 static_assert(sizeof(Barriers) <= 256, "barrier block too large");
-static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
 
 struct GemmParams {
-  const uint8_t* tiles;     // blob tiles
+  const uint8_t* tiles;     // blob boxes
   const float* sw;          // [Npad]
   const float* fb;          // [Npad]
   const float* scales;      // [T]
@@ -116,148 +134,209 @@ __device__ __forceinline__ uint32_t dequant_bf16(int32_t acc, float st, float sw
 }
 
 // ------------------------------------------------------------------------------ the kernel
+// CG = 1: one CTA per tile of 128 x BN;  CG = 2: a CTA pair per tile of 256 x BN.
+template <int CG>
 __global__ void __launch_bounds__(kNumThreads, 1)
 w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
+  using C = Cfg<CG>;
   extern __shared__ uint8_t smem_raw[];
   // SWIZZLE_128B operands need 1024-byte alignment
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
-  const uint32_t unpacked0 = smem_base;                                   // kUStages x 48 KB
-  const uint32_t packed0 = smem_base + kUStages * kUnpackedStage;         // kPStages x 24 KB
-  uint8_t* packed_ptr = smem + kUStages * kUnpackedStage;
+  const uint32_t unpacked0 = smem_base;
+  const uint32_t packed0 = smem_base + kStages * C::kUnpackedStage;
   uint8_t* unpacked_ptr = smem;
-  Barriers* bars = reinterpret_cast<Barriers*>(smem + kUStages * kUnpackedStage +
-                                               kPStages * kPackedStage);
+  uint8_t* packed_ptr = smem + kStages * C::kUnpackedStage;
+  Barriers* bars = reinterpret_cast<Barriers*>(packed_ptr + kPStages * C::kPackedStage);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
+  const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
+  const bool leader = rank == 0;
 
   if (warp == kProducerWarp && lane == 0) {
     ptx::prefetch_tensormap(&tmap_a);
     for (int i = 0; i < kPStages; ++i) {
       ptx::mbar_init(ptx::smem_u32(&bars->pfull[i]), 1);
-      ptx::mbar_init(ptx::smem_u32(&bars->pempty[i]), kNumUnpackWarps);
+      ptx::mbar_init(ptx::smem_u32(&bars->pempty[i]), kNumUnpackWarps + 4);
     }
-    for (int i = 0; i < kUStages; ++i) {
-      ptx::mbar_init(ptx::smem_u32(&bars->ufull[i]), kNumUnpackWarps);
-      ptx::mbar_init(ptx::smem_u32(&bars->uempty[i]), 1);
+    for (int i = 0; i < kStages; ++i) {
+      ptx::mbar_init(ptx::smem_u32(&bars->full[i]), C::kFullCount);
+      ptx::mbar_init(ptx::smem_u32(&bars->empty[i]), 1);
     }
     for (int i = 0; i < kAccStages; ++i) {
       ptx::mbar_init(ptx::smem_u32(&bars->tfull[i]), 1);
-      ptx::mbar_init(ptx::smem_u32(&bars->tempty[i]), 4);
+      ptx::mbar_init(ptx::smem_u32(&bars->tempty[i]), C::kTemptyCount);
     }
     ptx::fence_barrier_init();
   }
   if (warp == kMmaWarp) {
-    ptx::tmem_alloc<kTmemCols>(ptx::smem_u32(&bars->tmem_base));
+    if (CG == 2) ptx::tmem_alloc_2cta<kTmemCols>(ptx::smem_u32(&bars->tmem_base));
+    else ptx::tmem_alloc<kTmemCols>(ptx::smem_u32(&bars->tmem_base));
   }
   ptx::tcgen05_fence_before();
   __syncthreads();
+  if (CG == 2) ptx::cluster_sync_all();       // peer barriers initialised before any remote arrive
   ptx::tcgen05_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
 
   const int num_tiles = p.num_m * p.num_n;
+  const int first_tile = static_cast<int>(blockIdx.x) / CG;
+  const int tile_step = static_cast<int>(gridDim.x) / CG;
 
   if (warp == kProducerWarp) {
-    // ===================================================================== TMA producer
+    // ===================================================================== B producer (bulk TMA)
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
         const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
-        const uint8_t* b0 = p.tiles + static_cast<size_t>(2 * n_blk) * p.num_kb * kTileBytes;
-        const uint8_t* b1 = b0 + static_cast<size_t>(p.num_kb) * kTileBytes;
+        const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM;
+        // row groups of kTileRows rows: this CTA streams CG == 2 ? one : both of the tile's groups
+        const uint8_t* g0 = p.tiles + static_cast<size_t>(2 * n_blk + (CG == 2 ? rank : 0)) *
+                                          p.num_kb * kTileBytes;
         for (int kb = 0; kb < p.num_kb; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&bars->pempty[stage]), phase ^ 1u);
           const uint32_t full = ptx::smem_u32(&bars->pfull[stage]);
-          const uint32_t dst = packed0 + stage * kPackedStage;
-          ptx::mbar_arrive_expect_tx(full, kPackedStage);
-          ptx::tma_load_2d(dst, &tmap_a, kb * (BK / 2), m_blk * BM, full);
-          ptx::bulk_load_1d(dst + kPackedA, b0 + static_cast<size_t>(kb) * kTileBytes,
-                            kTileBytes, full);
-          ptx::bulk_load_1d(dst + kPackedA + kTileBytes, b1 + static_cast<size_t>(kb) * kTileBytes,
-                            kTileBytes, full);
+          const uint32_t dst = packed0 + stage * C::kPackedStage;
+          ptx::mbar_arrive_expect_tx(full, C::kPackedStage);
+          // A: 128 rows x 64 B of codes, SWIZZLE_64B; rows beyond T are zero-filled by TMA
+          ptx::tma_load_2d(dst, &tmap_a, kb * (BK / 2), row0, full);
+          ptx::bulk_load_1d(dst + kPackedA, g0 + static_cast<size_t>(kb) * kTileBytes, kTileBytes,
+                            full);
+          if (CG == 1) {
+            ptx::bulk_load_1d(dst + kPackedA + kTileBytes,
+                              g0 + static_cast<size_t>(p.num_kb + kb) * kTileBytes, kTileBytes, full);
+          }
           advance(stage, phase, kPStages);
         }
       }
     }
   } else if (warp == kMmaWarp) {
     // ===================================================================== MMA issuer
-    if (lane == 0) {
-      constexpr uint32_t idesc = ptx::make_idesc_i8(BM, BN);
+    if (leader && lane == 0) {
+      constexpr uint32_t idesc = ptx::make_idesc_i8(BM * CG, BN);
       int stage = 0, as = 0;
       uint32_t phase = 0, aphase = 0;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
         ptx::mbar_wait(ptx::smem_u32(&bars->tempty[as]), aphase ^ 1u);
         ptx::tcgen05_fence_after();
         const uint32_t tmem_d = tmem_base + as * BN;
         for (int kb = 0; kb < p.num_kb; ++kb) {
-          ptx::mbar_wait(ptx::smem_u32(&bars->ufull[stage]), phase);
+          ptx::mbar_wait(ptx::smem_u32(&bars->full[stage]), phase);
           ptx::tcgen05_fence_after();
-          const uint32_t a_addr = unpacked0 + stage * kUnpackedStage;
-          const uint32_t b_addr = a_addr + kUnpackedA;
+          const uint32_t a_col = tmem_base + kACol0 + stage * (BK / 4);
+          const uint32_t b_addr = unpacked0 + stage * C::kUnpackedStage;
 #pragma unroll
           for (int k = 0; k < BK / 32; ++k) {
-            const uint64_t da = ptx::make_smem_desc_sw128(a_addr + k * 32);
             const uint64_t db = ptx::make_smem_desc_sw128(b_addr + k * 32);
-            ptx::mma_i8_ss(tmem_d, da, db, idesc, (kb | k) != 0 ? 1u : 0u);
+            const uint32_t accum = (kb | k) != 0 ? 1u : 0u;
+            if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db, idesc, accum);
+            else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db, idesc, accum);
           }
-          ptx::tcgen05_commit(ptx::smem_u32(&bars->uempty[stage]));    // frees the smem stage
-          advance(stage, phase, kUStages);
+          // frees the operand stage (A columns + B smem) in every CTA of the pair
+          if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
+          else ptx::tcgen05_commit(ptx::smem_u32(&bars->empty[stage]));
+          advance(stage, phase, kStages);
         }
-        ptx::tcgen05_commit(ptx::smem_u32(&bars->tfull[as]));          // accumulator ready
+        if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->tfull[as]), 3);
+        else ptx::tcgen05_commit(ptx::smem_u32(&bars->tfull[as]));
         advance(as, aphase, kAccStages);
       }
     }
   } else if (warp >= kUnpackWarp0) {
-    // ===================================================================== int4 -> int8 unpack
-    const int uw = warp - kUnpackWarp0;                 // 0..7
+    // ===================================================================== B: int4 -> int8
+    const int ut = threadIdx.x - kUnpackWarp0 * 32;      // 0..127
     int ps = 0, us = 0;
     uint32_t pphase = 0, uphase = 0;
-    const int rsub = lane >> 2, c = lane & 3;           // row in 8-row group, 16-byte chunk
-    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    constexpr int kTasks = C::kBRows * 4 / (kNumUnpackWarps * 32);   // 16-byte chunks per thread
+    static_assert(C::kBRows * 4 % (kNumUnpackWarps * 32) == 0, "unpack tasks");
+    const uint32_t full_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->full[0]), 0);
+    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
       for (int kb = 0; kb < p.num_kb; ++kb) {
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
-        ptx::mbar_wait(ptx::smem_u32(&bars->uempty[us]), uphase ^ 1u);
-        const uint8_t* src = packed_ptr + ps * kPackedStage;
-        uint8_t* dst = unpacked_ptr + us * kUnpackedStage;
-        // 384 rows (A 128 + B 256) = 48 groups of 8 rows; warp uw takes groups uw, uw+8, ...
-        uint4 v[6];
+        const uint8_t* src = packed_ptr + ps * C::kPackedStage + kPackedA;
+        uint4 v[kTasks];
 #pragma unroll
-        for (int i = 0; i < 6; ++i) {
-          const int rg = uw + i * kNumUnpackWarps;
-          v[i] = *reinterpret_cast<const uint4*>(src + rg * 512 + lane * 16);
-        }
+        for (int i = 0; i < kTasks; ++i)
+          v[i] = *reinterpret_cast<const uint4*>(src + (ut + i * 128) * 16);
+        ptx::mbar_wait(ptx::smem_u32(&bars->empty[us]), uphase ^ 1u);
+        uint8_t* dst = unpacked_ptr + us * C::kUnpackedStage;
 #pragma unroll
-        for (int i = 0; i < 6; ++i) {
-          const int rg = uw + i * kNumUnpackWarps;
+        for (int i = 0; i < kTasks; ++i) {
+          const int task = ut + i * 128;
+          const int row = task >> 2, c = task & 3, rsub = row & 7;
           uint4 lo, hi;
           lo.x = (v[i].x << 4) & 0xF0F0F0F0u; hi.x = v[i].x & 0xF0F0F0F0u;
           lo.y = (v[i].y << 4) & 0xF0F0F0F0u; hi.y = v[i].y & 0xF0F0F0F0u;
           lo.z = (v[i].z << 4) & 0xF0F0F0F0u; hi.z = v[i].z & 0xF0F0F0F0u;
           lo.w = (v[i].w << 4) & 0xF0F0F0F0u; hi.w = v[i].w & 0xF0F0F0F0u;
-          uint8_t* row = dst + rg * 1024 + rsub * 128;
-          *reinterpret_cast<uint4*>(row + (((2 * c) ^ rsub) << 4)) = lo;
-          *reinterpret_cast<uint4*>(row + (((2 * c + 1) ^ rsub) << 4)) = hi;
+          uint8_t* rp = dst + row * 128;                  // 8-row swizzle atoms of 1024 bytes
+          *reinterpret_cast<uint4*>(rp + (((2 * c) ^ rsub) << 4)) = lo;
+          *reinterpret_cast<uint4*>(rp + (((2 * c + 1) ^ rsub) << 4)) = hi;
         }
         ptx::fence_proxy_async_smem();      // generic-proxy writes -> visible to tcgen05.mma
         __syncwarp();
         if (lane == 0) {
-          ptx::mbar_arrive(ptx::smem_u32(&bars->ufull[us]));
+          ptx::mbar_arrive(ptx::smem_u32(&bars->pempty[ps]));
+          ptx::mbar_arrive_cluster(full_remote + us * 8);
+        }
+        advance(ps, pphase, kPStages);
+        advance(us, uphase, kStages);
+      }
+    }
+  } else if (warp >= kAWarp0 && warp < kAWarp0 + 4) {
+    // ===================================================================== A: smem -> TMEM
+    // thread = token row = TMEM lane.  The packed tile is [128 rows][64 B] with TMA's SWIZZLE_64B
+    // (16-byte chunk index ^= (row >> 1) & 3), so the 32 lanes' 16-byte reads of one chunk column
+    // spread over all banks (4 wavefronts per 512 B: the minimum).
+    const int q = warp & 3;                               // TMEM lane quarter
+    const int arow = q * 32 + lane;
+    const uint32_t full_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->full[0]), 0);
+    const uint32_t a_taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + kACol0;
+    const int sw = (arow >> 1) & 3;
+    int ps = 0, us = 0;
+    uint32_t pphase = 0, uphase = 0;
+    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
+      for (int kb = 0; kb < p.num_kb; ++kb) {
+        ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
+        const uint8_t* src = packed_ptr + ps * C::kPackedStage + arow * 64;
+        uint4 w4[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) w4[c] = *reinterpret_cast<const uint4*>(src + ((c ^ sw) << 4));
+        uint32_t r[32];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const uint4 w = w4[c];
+          r[8 * c + 0] = (w.x << 4) & 0xF0F0F0F0u; r[8 * c + 4] = w.x & 0xF0F0F0F0u;
+          r[8 * c + 1] = (w.y << 4) & 0xF0F0F0F0u; r[8 * c + 5] = w.y & 0xF0F0F0F0u;
+          r[8 * c + 2] = (w.z << 4) & 0xF0F0F0F0u; r[8 * c + 6] = w.z & 0xF0F0F0F0u;
+          r[8 * c + 3] = (w.w << 4) & 0xF0F0F0F0u; r[8 * c + 7] = w.w & 0xF0F0F0F0u;
+        }
+        ptx::mbar_wait(ptx::smem_u32(&bars->empty[us]), uphase ^ 1u);
+        ptx::tcgen05_fence_after();
+        ptx::tmem_st_32x32b_x32(a_taddr + us * (BK / 4), r);
+        ptx::tmem_st_wait();
+        ptx::tcgen05_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          ptx::mbar_arrive_cluster(full_remote + us * 8);
+          // the store consumed every lane's smem reads: the packed stage may be refilled
           ptx::mbar_arrive(ptx::smem_u32(&bars->pempty[ps]));
         }
         advance(ps, pphase, kPStages);
-        advance(us, uphase, kUStages);
+        advance(us, uphase, kStages);
       }
     }
   } else if (warp >= kEpiWarp0 && warp < kEpiWarp0 + 4) {
     // ===================================================================== epilogue
     const int q = warp & 3;                             // TMEM lane quarter
+    const uint32_t tempty_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->tempty[0]), 0);
     int as = 0;
     uint32_t aphase = 0;
-    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
       const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
-      const int row = m_blk * BM + q * 32 + lane;
+      const int row = m_blk * (BM * CG) + static_cast<int>(rank) * BM + q * 32 + lane;
       const bool row_ok = row < p.T;
       const float st = row_ok ? p.scales[row] : 0.0f;
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
@@ -304,21 +383,28 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       // all TMEM reads of this warp are complete (wait::ld above): release the accumulator
       ptx::tcgen05_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&bars->tempty[as]));
+      if (lane == 0) ptx::mbar_arrive_cluster(tempty_remote + as * 8);
       advance(as, aphase, kAccStages);
     }
   }
 
-  // ---- teardown
+  // ---- teardown: nobody leaves while the peer may still touch this CTA's barriers / smem
   ptx::tcgen05_fence_before();
   __syncthreads();
+  if (CG == 2) ptx::cluster_sync_all();
   if (warp == kMmaWarp) {
     ptx::tcgen05_fence_after();
-    ptx::tmem_dealloc<kTmemCols>(tmem_base);
+    if (CG == 2) ptx::tmem_dealloc_2cta<kTmemCols>(tmem_base);
+    else ptx::tmem_dealloc<kTmemCols>(tmem_base);
   }
 }
 
+}  // namespace
+
+
 // ------------------------------------------------------------------------------ host side
+namespace {
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -338,28 +424,59 @@ EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
+template <int CG>
+cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sms,
+                      cudaStream_t stream) {
+  using C = Cfg<CG>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(w4a4_gemm_kernel<CG>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const int tiles = p.num_m * p.num_n;
+  const int slots = num_sms / CG;                        // CTAs (CG = 1) or CTA pairs (CG = 2)
+  const int groups = tiles < slots ? tiles : slots;
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(static_cast<unsigned>(groups * CG), 1, 1);
+  cfg.blockDim = dim3(kNumThreads, 1, 1);
+  cfg.dynamicSmemBytes = C::kSmemBytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CG;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG>, tmap_a, p);
+}
+
 }  // namespace
 
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
-  if (g.x != nullptr) return cudaErrorNotSupported;     // fused producer: separate kernel (TODO)
+  if (g.x != nullptr) return cudaErrorNotSupported;     // fused producer: see launch_w4a4_fused
+  const BlobHeader h = blob_header(g.N, g.K);
+  const uint8_t* base = static_cast<const uint8_t*>(g.blob);
+  const int cg = g.cta_group == 1 ? 1 : 2;
   EncodeTiledFn encode = get_encode_fn();
   if (encode == nullptr) return cudaErrorNotSupported;
 
-  const BlobHeader h = blob_header(g.N, g.K);
-  const uint8_t* base = static_cast<const uint8_t*>(g.blob);
-
-  // A operand: codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows; rows beyond T are
-  // zero-filled by TMA, so a ragged last M tile needs no special case in the main loop.
-  CUtensorMap tmap;
-  const cuuint64_t dims[2] = {static_cast<cuuint64_t>(g.K / 2), static_cast<cuuint64_t>(g.T)};
-  const cuuint64_t strides[1] = {static_cast<cuuint64_t>(g.K / 2)};
-  const cuuint32_t box[2] = {static_cast<cuuint32_t>(BK / 2), static_cast<cuuint32_t>(BM)};
-  const cuuint32_t estr[2] = {1, 1};
-  const CUresult r = encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
-                            const_cast<uint8_t*>(g.codes), dims, strides, box, estr,
-                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  // A operand: codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows, SWIZZLE_64B; rows
+  // beyond T are zero-filled by TMA, so a ragged last M tile needs no special case.
+  CUtensorMap tmap_a;
+  {
+    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(g.K / 2), static_cast<cuuint64_t>(g.T)};
+    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(g.K / 2)};
+    const cuuint32_t box[2] = {static_cast<cuuint32_t>(BK / 2), static_cast<cuuint32_t>(BM)};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(&tmap_a, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
+                              const_cast<uint8_t*>(g.codes), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  }
 
   GemmParams p;
   p.tiles = base + h.off_tiles;
@@ -372,21 +489,11 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   p.T = g.T;
   p.N = g.N;
   p.K = g.K;
-  p.num_m = (g.T + BM - 1) / BM;
+  p.num_m = (g.T + BM * cg - 1) / (BM * cg);
   p.num_n = h.Npad / BN;
   p.num_kb = g.K / BK;
-
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(w4a4_gemm_kernel,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
-  const int tiles = p.num_m * p.num_n;
-  const int grid = tiles < g.num_sms ? tiles : g.num_sms;
-  w4a4_gemm_kernel<<<grid, kNumThreads, kSmemBytes, g.stream>>>(tmap, p);
-  return cudaGetLastError();
+  return cg == 2 ? launch_cg<2>(tmap_a, p, g.num_sms, g.stream)
+                 : launch_cg<1>(tmap_a, p, g.num_sms, g.stream);
 }
 
 }  // namespace baseq
