@@ -40,7 +40,7 @@ constexpr int BM = 128;                 // token rows per CTA (TMEM lanes)
 constexpr int BN = kGemmBN;             // output channels per tile (UMMA N)
 constexpr int BK = 128;                 // int4 elements along K per stage
 constexpr int kStages = 4;              // operand stages: A in TMEM (32 columns), B unpacked in smem
-constexpr int kPStages = 4;             // packed-B ring
+constexpr int kPStagesMax = 8;          // packed ring depth (TMA latency from L2 is ~1.5k clk)
 constexpr int kAccStages = 2;
 constexpr int kACol0 = kAccStages * BN; // first TMEM column of the A stages
 constexpr int kTmemCols = 512;
@@ -48,13 +48,18 @@ constexpr int kPackedA = BM * BK / 2;    // 8 KB of packed codes per CTA and k-b
 static_assert(kACol0 + kStages * (BK / 4) <= kTmemCols, "TMEM budget");
 static_assert(BN % 32 == 0 && BN <= 256, "UMMA N");
 
-constexpr int kNumThreads = 512;
-constexpr int kProducerWarp = 0;
+constexpr int kNumThreads = 896;
+constexpr int kSets = 2;                // A and B warp sets alternate k-blocks: one warp's serial
+                                        // chain per k-block (two try_waits, LDS, expand, store,
+                                        // fence, arrive: 400-700 clk) exceeds the 384 clk MMA time
+constexpr int kProducerWarp = 0;        // A operand (tensor-map TMA)
+constexpr int kProducerWarpB = 2;       // B operand (bulk TMA)
 constexpr int kMmaWarp = 1;
-constexpr int kEpiWarp0 = 4;            // warps 4..7   (warp % 4 = TMEM lane quarter)
-constexpr int kAWarp0 = 8;              // warps 8..11  (warp % 4 = TMEM lane quarter)
-constexpr int kUnpackWarp0 = 12;        // warps 12..15
-constexpr int kNumUnpackWarps = 4;
+constexpr int kEpiWarp0 = 4;            // warps 4..11  (warp % 4 = TMEM lane quarter), 2 column halves
+constexpr int kEpiWarps = 8;
+constexpr int kAWarp0 = 12;             // warps 12..19 (warp % 4 = TMEM lane quarter), 2 sets
+constexpr int kUnpackWarp0 = 20;        // warps 20..27, 2 sets
+constexpr int kNumUnpackWarps = 4;      // per set
 
 template <int CG>
 struct Cfg {
@@ -63,12 +68,14 @@ struct Cfg {
   static constexpr int kPackedStage = kPackedA + kPackedB;  // multiple of 1024 (swizzle alignment)
   static constexpr int kUnpackedStage = kBRows * BK;
   static constexpr int kFullCount = CG * (4 + kNumUnpackWarps);
-  static constexpr int kTemptyCount = CG * 4;
+  static constexpr int kTemptyCount = CG * kEpiWarps;
+  static constexpr int kPStages = CG == 2 ? kPStagesMax : 5;
   static constexpr int kSmemBytes = 1024 + kStages * kUnpackedStage + kPStages * kPackedStage + 256;
+  static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
 };
 
 struct __align__(8) Barriers {
-  uint64_t pfull[kPStages], pempty[kPStages];   // packed-B ring, CTA-local
+  uint64_t pfull[kPStagesMax], pempty[kPStagesMax];   // packed-B ring, CTA-local
   uint64_t full[kStages];                       // operand stage ready   (waited on in the leader CTA)
   uint64_t empty[kStages];                      // operand stage free    (every CTA; MMA commit)
   uint64_t tfull[kAccStages];                   // accumulator ready     (every CTA; MMA commit)
@@ -116,8 +123,18 @@ __device__ __forceinline__ uint32_t bf16_from_double_rne(double v) {
   return r >> 16;
 }
 
+// One output.  Fast path: t = RN(s_t * accf), p = RN(t * s_w), y = RN(t * s_w + fb) and the
+// bracket [y - E, y + E] with E = 2^-23 (|p| + |y|) >= 2 |y - y*| (see above); when both ends round
+// to the same bf16 (all but ~2.4e-4 of the elements, whatever the cancellation between p and fb)
+// that is the result, otherwise the fp64 expression itself is evaluated.
+__device__ __noinline__ uint32_t dequant_f64(int32_t acc, float st, float sw, float fb) {
+  const double pd = __dmul_rn(static_cast<double>(st), static_cast<double>(sw));
+  const double yd = __fma_rn(pd, static_cast<double>(acc), static_cast<double>(fb));
+  return bf16_from_double_rne(yd);
+}
 __device__ __forceinline__ uint32_t dequant_bf16(int32_t acc, float st, float sw, float fb) {
-  const float accf = __int2float_rn(acc);                 // exact: |acc| < 2^24
+  // exact int -> float without the quarter-rate I2F: |acc| <= 64 K < 2^22
+  const float accf = __fsub_rn(__int_as_float(0x4B400000 + acc), 12582912.0f);
   const float t = __fmul_rn(st, accf);
   const float p = __fmul_rn(t, sw);
   const float y = __fmaf_rn(t, sw, fb);
@@ -128,9 +145,11 @@ __device__ __forceinline__ uint32_t dequant_bf16(int32_t acc, float st, float sw
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));   // hi -> upper half
   const uint32_t a = pk & 0xFFFFu, b = pk >> 16;
   if (a == b && fabsf(y) > 1e-30f) return a;
-  const double pd = __dmul_rn(static_cast<double>(st), static_cast<double>(sw));
-  const double yd = __fma_rn(pd, static_cast<double>(acc), static_cast<double>(fb));
-  return bf16_from_double_rne(yd);
+  return dequant_f64(acc, st, sw, fb);
+}
+__device__ __forceinline__ uint32_t dequant_bf16x2(int32_t a0, int32_t a1, float st, float2 sw,
+                                                   float2 fb) {
+  return dequant_bf16(a0, st, sw.x, fb.x) | (dequant_bf16(a1, st, sw.y, fb.y) << 16);
 }
 
 // ------------------------------------------------------------------------------ the kernel
@@ -147,7 +166,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
   const uint32_t packed0 = smem_base + kStages * C::kUnpackedStage;
   uint8_t* unpacked_ptr = smem;
   uint8_t* packed_ptr = smem + kStages * C::kUnpackedStage;
-  Barriers* bars = reinterpret_cast<Barriers*>(packed_ptr + kPStages * C::kPackedStage);
+  Barriers* bars = reinterpret_cast<Barriers*>(packed_ptr + C::kPStages * C::kPackedStage);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -156,8 +175,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
 
   if (warp == kProducerWarp && lane == 0) {
     ptx::prefetch_tensormap(&tmap_a);
-    for (int i = 0; i < kPStages; ++i) {
-      ptx::mbar_init(ptx::smem_u32(&bars->pfull[i]), 1);
+    for (int i = 0; i < C::kPStages; ++i) {
+      ptx::mbar_init(ptx::smem_u32(&bars->pfull[i]), 2);
       ptx::mbar_init(ptx::smem_u32(&bars->pempty[i]), kNumUnpackWarps + 4);
     }
     for (int i = 0; i < kStages; ++i) {
@@ -184,40 +203,54 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
   const int first_tile = static_cast<int>(blockIdx.x) / CG;
   const int tile_step = static_cast<int>(gridDim.x) / CG;
 
-  if (warp == kProducerWarp) {
-    // ===================================================================== B producer (bulk TMA)
-    if (lane == 0) {
-      int stage = 0;
-      uint32_t phase = 0;
-      for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-        const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
-        const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM;
-        // row groups of kTileRows rows: this CTA streams CG == 2 ? one : both of the tile's groups
-        const uint8_t* g0 = p.tiles + static_cast<size_t>(2 * n_blk + (CG == 2 ? rank : 0)) *
-                                          p.num_kb * kTileBytes;
-        for (int kb = 0; kb < p.num_kb; ++kb) {
-          ptx::mbar_wait(ptx::smem_u32(&bars->pempty[stage]), phase ^ 1u);
-          const uint32_t full = ptx::smem_u32(&bars->pfull[stage]);
-          const uint32_t dst = packed0 + stage * C::kPackedStage;
-          ptx::mbar_arrive_expect_tx(full, C::kPackedStage);
-          // A: 128 rows x 64 B of codes, SWIZZLE_64B; rows beyond T are zero-filled by TMA
-          ptx::tma_load_2d(dst, &tmap_a, kb * (BK / 2), row0, full);
-          ptx::bulk_load_1d(dst + kPackedA, g0 + static_cast<size_t>(kb) * kTileBytes, kTileBytes,
-                            full);
-          if (CG == 1) {
-            ptx::bulk_load_1d(dst + kPackedA + kTileBytes,
-                              g0 + static_cast<size_t>(p.num_kb + kb) * kTileBytes, kTileBytes, full);
+  if (warp == kProducerWarp || warp == kProducerWarpB) {
+    // ===================================================================== producers (TMA)
+    // Two warps, one per operand: a single warp's wait + expect_tx + two copy issues per k-block
+    // is a ~350 clk serial chain (measured with everything else stubbed out).
+    const bool is_a = warp == kProducerWarp;
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
+      const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
+      const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM;
+      // row groups of kTileRows rows: this CTA streams CG == 2 ? one : both of the tile's groups
+      const uint8_t* g0 = p.tiles + static_cast<size_t>(2 * n_blk + (CG == 2 ? rank : 0)) *
+                                        p.num_kb * kTileBytes;
+      for (int kb = 0; kb < p.num_kb; ++kb) {
+        ptx::mbar_wait(ptx::smem_u32(&bars->pempty[stage]), phase ^ 1u);
+        const uint32_t full = ptx::smem_u32(&bars->pfull[stage]);
+        const uint32_t dst = packed0 + stage * C::kPackedStage;
+        if (ptx::elect_one()) {
+          if (is_a) {
+            // A: 128 rows x 64 B of codes, SWIZZLE_64B; rows beyond T are zero-filled by TMA
+            ptx::mbar_arrive_expect_tx(full, kPackedA);
+            ptx::tma_load_2d(dst, &tmap_a, kb * (BK / 2), row0, full);
+          } else {
+            ptx::mbar_arrive_expect_tx(full, C::kPackedB);
+            ptx::bulk_load_1d(dst + kPackedA, g0 + static_cast<size_t>(kb) * kTileBytes,
+                              kTileBytes, full);
+            if (CG == 1) {
+              ptx::bulk_load_1d(dst + kPackedA + kTileBytes,
+                                g0 + static_cast<size_t>(p.num_kb + kb) * kTileBytes, kTileBytes,
+                                full);
+            }
           }
-          advance(stage, phase, kPStages);
         }
+        __syncwarp();
+        advance(stage, phase, C::kPStages);
       }
     }
   } else if (warp == kMmaWarp) {
     // ===================================================================== MMA issuer
-    if (leader && lane == 0) {
+    // The whole warp runs the loop in uniform control flow and one elected lane issues: with a
+    // divergent `lane == 0` region ptxas wraps every tcgen05 instruction in a vote/elect/R2UR
+    // waterfall (~95 SASS instructions and ~670 clk per k-block, measured -- slower than the
+    // 384 clk the four MMAs take).
+    if (leader) {
       constexpr uint32_t idesc = ptx::make_idesc_i8(BM * CG, BN);
       int stage = 0, as = 0;
       uint32_t phase = 0, aphase = 0;
+      const uint64_t desc0 = ptx::make_smem_desc_sw128(unpacked0);
       for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
         ptx::mbar_wait(ptx::smem_u32(&bars->tempty[as]), aphase ^ 1u);
         ptx::tcgen05_fence_after();
@@ -225,35 +258,48 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
         for (int kb = 0; kb < p.num_kb; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&bars->full[stage]), phase);
           ptx::tcgen05_fence_after();
-          const uint32_t a_col = tmem_base + kACol0 + stage * (BK / 4);
-          const uint32_t b_addr = unpacked0 + stage * C::kUnpackedStage;
+          if (ptx::elect_one()) {
+            const uint32_t a_col = tmem_base + kACol0 + stage * (BK / 4);
+            // descriptor start-address field is in 16-byte units: + stage bytes/16, + 2 per K chunk
+            const uint64_t db = desc0 + static_cast<uint64_t>(stage * (C::kUnpackedStage >> 4));
 #pragma unroll
-          for (int k = 0; k < BK / 32; ++k) {
-            const uint64_t db = ptx::make_smem_desc_sw128(b_addr + k * 32);
-            const uint32_t accum = (kb | k) != 0 ? 1u : 0u;
-            if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db, idesc, accum);
-            else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db, idesc, accum);
+            for (int k = 0; k < BK / 32; ++k) {
+              const uint32_t accum = (kb | k) != 0 ? 1u : 0u;
+              if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+              else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+            }
+            // frees the operand stage (A columns + B smem) in every CTA of the pair
+            if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
+            else ptx::tcgen05_commit(ptx::smem_u32(&bars->empty[stage]));
           }
-          // frees the operand stage (A columns + B smem) in every CTA of the pair
-          if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
-          else ptx::tcgen05_commit(ptx::smem_u32(&bars->empty[stage]));
+          __syncwarp();
           advance(stage, phase, kStages);
         }
-        if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->tfull[as]), 3);
-        else ptx::tcgen05_commit(ptx::smem_u32(&bars->tfull[as]));
+        if (ptx::elect_one()) {
+          if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->tfull[as]), 3);
+          else ptx::tcgen05_commit(ptx::smem_u32(&bars->tfull[as]));
+        }
+        __syncwarp();
         advance(as, aphase, kAccStages);
       }
     }
-  } else if (warp >= kUnpackWarp0) {
+  } else if (warp >= kUnpackWarp0 && warp < kUnpackWarp0 + kNumUnpackWarps * kSets) {
     // ===================================================================== B: int4 -> int8
-    const int ut = threadIdx.x - kUnpackWarp0 * 32;      // 0..127
+    const int ut = (threadIdx.x - kUnpackWarp0 * 32) & 127;   // 0..127 inside the set
+    const int set = (warp - kUnpackWarp0) >> 2;
+    int it = 0;
     int ps = 0, us = 0;
     uint32_t pphase = 0, uphase = 0;
     constexpr int kTasks = C::kBRows * 4 / (kNumUnpackWarps * 32);   // 16-byte chunks per thread
     static_assert(C::kBRows * 4 % (kNumUnpackWarps * 32) == 0, "unpack tasks");
     const uint32_t full_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->full[0]), 0);
     for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-      for (int kb = 0; kb < p.num_kb; ++kb) {
+      for (int kb = 0; kb < p.num_kb; ++kb, ++it) {
+        if ((it & (kSets - 1)) != set) {
+          advance(ps, pphase, C::kPStages);
+          advance(us, uphase, kStages);
+          continue;
+        }
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
         const uint8_t* src = packed_ptr + ps * C::kPackedStage + kPackedA;
         uint4 v[kTasks];
@@ -281,11 +327,11 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           ptx::mbar_arrive(ptx::smem_u32(&bars->pempty[ps]));
           ptx::mbar_arrive_cluster(full_remote + us * 8);
         }
-        advance(ps, pphase, kPStages);
+        advance(ps, pphase, C::kPStages);
         advance(us, uphase, kStages);
       }
     }
-  } else if (warp >= kAWarp0 && warp < kAWarp0 + 4) {
+  } else if (warp >= kAWarp0 && warp < kAWarp0 + 4 * kSets) {
     // ===================================================================== A: smem -> TMEM
     // thread = token row = TMEM lane.  The packed tile is [128 rows][64 B] with TMA's SWIZZLE_64B
     // (16-byte chunk index ^= (row >> 1) & 3), so the 32 lanes' 16-byte reads of one chunk column
@@ -295,10 +341,17 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     const uint32_t full_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->full[0]), 0);
     const uint32_t a_taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + kACol0;
     const int sw = (arow >> 1) & 3;
+    const int set = (warp - kAWarp0) >> 2;
+    int it = 0;
     int ps = 0, us = 0;
     uint32_t pphase = 0, uphase = 0;
     for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-      for (int kb = 0; kb < p.num_kb; ++kb) {
+      for (int kb = 0; kb < p.num_kb; ++kb, ++it) {
+        if ((it & (kSets - 1)) != set) {
+          advance(ps, pphase, C::kPStages);
+          advance(us, uphase, kStages);
+          continue;
+        }
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
         const uint8_t* src = packed_ptr + ps * C::kPackedStage + arow * 64;
         uint4 w4[4];
@@ -324,13 +377,17 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           // the store consumed every lane's smem reads: the packed stage may be refilled
           ptx::mbar_arrive(ptx::smem_u32(&bars->pempty[ps]));
         }
-        advance(ps, pphase, kPStages);
+        advance(ps, pphase, C::kPStages);
         advance(us, uphase, kStages);
       }
     }
-  } else if (warp >= kEpiWarp0 && warp < kEpiWarp0 + 4) {
+  } else if (warp >= kEpiWarp0 && warp < kEpiWarp0 + kEpiWarps) {
     // ===================================================================== epilogue
-    const int q = warp & 3;                             // TMEM lane quarter
+    // 8 warps: warp % 4 = TMEM lane quarter (32 token rows), (warp - kEpiWarp0) / 4 = which half
+    // of the tile's BN columns.  16 columns per tcgen05.ld keep the register footprint small.
+    const int q = warp & 3;
+    const int half = (warp - kEpiWarp0) >> 2;
+    constexpr int kColsPerWarp = BN / (kEpiWarps / 4);
     const uint32_t tempty_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->tempty[0]), 0);
     int as = 0;
     uint32_t aphase = 0;
@@ -341,17 +398,19 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       const float st = row_ok ? p.scales[row] : 0.0f;
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
       ptx::tcgen05_fence_after();
-      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN;
-      const int n0 = n_blk * BN;
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN +
+                             half * kColsPerWarp;
+      const int n0 = n_blk * BN + half * kColsPerWarp;
+      uint16_t* yrow = p.y + static_cast<int64_t>(row) * p.ldy;
 #pragma unroll 1
-      for (int c0 = 0; c0 < BN; c0 += 32) {
+      for (int c0 = 0; c0 < kColsPerWarp; c0 += 16) {
         if (n0 + c0 >= p.N) break;                      // warp-uniform
-        uint32_t r[32];
-        ptx::tmem_ld_32x32b_x32(taddr + c0, r);
+        uint32_t r[16];
+        ptx::tmem_ld_32x32b_x16(taddr + c0, r);
         ptx::tmem_ld_wait();
-        uint32_t out[16];
+        uint32_t out[8];
 #pragma unroll
-        for (int j = 0; j < 32; j += 2) {
+        for (int j = 0; j < 16; j += 2) {
           const int n = n0 + c0 + j;
           const int32_t a0 = static_cast<int32_t>(r[j]) >> 8;       // raw = 256 * acc
           const int32_t a1 = static_cast<int32_t>(r[j + 1]) >> 8;
@@ -359,16 +418,14 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           r[j + 1] = static_cast<uint32_t>(a1);
           const float2 sw = __ldg(reinterpret_cast<const float2*>(p.sw + n));
           const float2 fb = __ldg(reinterpret_cast<const float2*>(p.fb + n));
-          const uint32_t y0 = dequant_bf16(a0, st, sw.x, fb.x);
-          const uint32_t y1 = dequant_bf16(a1, st, sw.y, fb.y);
-          out[j >> 1] = y0 | (y1 << 16);
+          out[j >> 1] = dequant_bf16x2(a0, a1, st, sw, fb);
         }
         if (row_ok) {
 #pragma unroll
-          for (int g = 0; g < 4; ++g) {
+          for (int g = 0; g < 2; ++g) {
             const int n = n0 + c0 + g * 8;
             if (n < p.N) {
-              *reinterpret_cast<uint4*>(p.y + static_cast<int64_t>(row) * p.ldy + n) =
+              *reinterpret_cast<uint4*>(yrow + n) =
                   make_uint4(out[4 * g], out[4 * g + 1], out[4 * g + 2], out[4 * g + 3]);
               if (p.acc_dump != nullptr) {
                 int32_t* d = p.acc_dump + static_cast<int64_t>(row) * p.N + n;
