@@ -265,6 +265,18 @@ __device__ __forceinline__ void mma_i8_ts_2cta(uint32_t tmem_d, uint32_t tmem_a,
       ::"r"(tmem_d), "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+// CTA-pair .ss form: both operands from shared-memory descriptors (each CTA's own A rows, half of B)
+__device__ __forceinline__ void mma_i8_ss_2cta(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b,
+                                               uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t"
+      "}\n"
+      ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
 // commit -> arrive on the mbarrier at this offset in every CTA of `cta_mask`
 __device__ __forceinline__ void tcgen05_commit_2cta(uint32_t bar, uint16_t cta_mask) {
   asm volatile(

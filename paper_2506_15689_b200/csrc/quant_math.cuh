@@ -1,0 +1,112 @@
+// The quantiser's arithmetic contract (Q0-Q7), written once and used by
+// both the stand-alone row kernel (quantize_act.cu) and the quantise-in-producer warps of the
+// fused GEMM (w4a4_gemm.cu).  Every line is one correctly rounded fp32 operation -- explicit
+// __f*_rn intrinsics are never contracted or re-associated by nvcc.
+//
+// Unit of work: one 16-byte vector = 8 consecutive bf16 channels of one token, held by one lane;
+// the 16 lanes of an aligned half-warp hold 128 consecutive channels (vector index = lane & 15 in
+// the fused GEMM, any aligned run of consecutive vectors in the row kernel).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace baseq {
+namespace qm {
+
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
+
+// Q0: bf16 -> fp32 (exact)
+__device__ __forceinline__ void unpack8(const uint4& v, float (&f)[8]) {
+  f[0] = bf16_lo(v.x); f[1] = bf16_hi(v.x);
+  f[2] = bf16_lo(v.y); f[3] = bf16_hi(v.y);
+  f[4] = bf16_lo(v.z); f[5] = bf16_hi(v.z);
+  f[6] = bf16_lo(v.w); f[7] = bf16_hi(v.w);
+}
+
+// Q1: block Hadamard over had_block channels (power of two, <= 256), increasing-stride Sylvester
+// butterflies (a, b) <- (a + b, a - b), then one multiply by (float)(1/sqrt(had_block)).
+// Strides 1, 2, 4 stay inside the lane's 8 channels; strides 8 .. B/2 pair lane l with lane
+// l ^ (stride / 8): the lower lane computes own + other, the upper other - own = fma(own, -1, other)
+// (the same single rounding as a - b).  Must be called by all 32 lanes.
+__device__ __forceinline__ void hadamard8(float (&f)[8], int had_block, float had_scale, int lane) {
+#pragma unroll
+  for (int h = 1; h < 8; h <<= 1) {
+    if (h < had_block) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if ((j & h) == 0) {
+          const float a = f[j], b2 = f[j + h];
+          f[j] = __fadd_rn(a, b2);
+          f[j + h] = __fsub_rn(a, b2);
+        }
+      }
+    }
+  }
+  for (int h = 8; h < had_block; h <<= 1) {
+    const int lm = h >> 3;
+    const float sgn = (lane & lm) ? -1.0f : 1.0f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const float other = __shfl_xor_sync(0xffffffffu, f[j], lm);
+      f[j] = __fmaf_rn(f[j], sgn, other);
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 8; ++j) f[j] = __fmul_rn(f[j], had_scale);
+}
+
+// Per-channel parameters of one vector: g = sa ? sa[k] : gamma, b = bvec ? bvec[k] : 0.
+__device__ __forceinline__ void load_gb(const float* __restrict__ sa, const float* __restrict__ bvec,
+                                        float gamma, int vec_idx, bool ok, float (&g)[8],
+                                        float (&bb)[8]) {
+  if (sa != nullptr && ok) {
+    const float4 g0 = __ldg(reinterpret_cast<const float4*>(sa) + 2 * vec_idx);
+    const float4 g1 = __ldg(reinterpret_cast<const float4*>(sa) + 2 * vec_idx + 1);
+    g[0] = g0.x; g[1] = g0.y; g[2] = g0.z; g[3] = g0.w;
+    g[4] = g1.x; g[5] = g1.y; g[6] = g1.z; g[7] = g1.w;
+  } else {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) g[j] = gamma;
+  }
+  if (bvec != nullptr && ok) {
+    const float4 b0 = __ldg(reinterpret_cast<const float4*>(bvec) + 2 * vec_idx);
+    const float4 b1 = __ldg(reinterpret_cast<const float4*>(bvec) + 2 * vec_idx + 1);
+    bb[0] = b0.x; bb[1] = b0.y; bb[2] = b0.z; bb[3] = b0.w;
+    bb[4] = b1.x; bb[5] = b1.y; bb[6] = b1.z; bb[7] = b1.w;
+  } else {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) bb[j] = 0.0f;
+  }
+}
+
+// Q2: u = fma(g, h, -b)
+__device__ __forceinline__ float affine(float g, float h, float b) { return __fmaf_rn(g, h, -b); }
+
+// Q4, Q5: per-token step size and its reciprocal
+__device__ __forceinline__ float step_size(float alpha, float absmax) {
+  return fmaxf(__fdiv_rn(__fmul_rn(alpha, absmax), 7.0f), 1e-12f);
+}
+__device__ __forceinline__ float reciprocal(float st) { return __fdiv_rn(1.0f, st); }
+
+// Q6: bits whose low nibble is the two's-complement code clamp(rne(u * inv), -8, 7)
+// (magic add: 1.5 * 2^23 + r has ulp 1, so the fp32 add performs the round-half-to-even).
+__device__ __forceinline__ uint32_t code_bits(float u, float inv) {
+  float r = __fmul_rn(u, inv);
+  r = fminf(fmaxf(r, -8.0f), 7.0f);
+  return __float_as_uint(__fadd_rn(r, 12582912.0f));
+}
+
+// Q7: 8 codes -> one 32-bit word of nibbles (channel j in nibble j)
+__device__ __forceinline__ uint32_t pack_nibbles(const uint32_t (&t)[8]) {
+  const uint32_t p0 = (t[0] & 0xFu) | (t[1] << 4);
+  const uint32_t p1 = (t[2] & 0xFu) | (t[3] << 4);
+  const uint32_t p2 = (t[4] & 0xFu) | (t[5] << 4);
+  const uint32_t p3 = (t[6] & 0xFu) | (t[7] << 4);
+  const uint32_t lo = __byte_perm(p0, p1, 0x0040);   // bytes: p0.b0, p1.b0, -, -
+  const uint32_t hi = __byte_perm(p2, p3, 0x0040);
+  return __byte_perm(lo, hi, 0x5410);                // lo.b0 lo.b1 hi.b0 hi.b1
+}
+
+}  // namespace qm
+}  // namespace baseq

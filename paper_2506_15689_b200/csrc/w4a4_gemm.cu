@@ -32,6 +32,7 @@
 
 #include "kernels.cuh"
 #include "ptx.cuh"
+#include "quant_math.cuh"
 
 namespace baseq {
 namespace {
@@ -48,29 +49,40 @@ constexpr int kPackedA = BM * BK / 2;    // 8 KB of packed codes per CTA and k-b
 static_assert(kACol0 + kStages * (BK / 4) <= kTmemCols, "TMEM budget");
 static_assert(BN % 32 == 0 && BN <= 256, "UMMA N");
 
-constexpr int kNumThreads = 896;
-constexpr int kSets = 2;                // A and B warp sets alternate k-blocks: one warp's serial
+constexpr int kSetsMax = 2;             // A and B warp sets alternate k-blocks: one warp's serial
                                         // chain per k-block (two try_waits, LDS, expand, store,
                                         // fence, arrive: 400-700 clk) exceeds the 384 clk MMA time
-constexpr int kProducerWarp = 0;        // A operand (tensor-map TMA)
+constexpr int kProducerWarp = 0;        // A operand (tensor-map TMA; idle in the fused variant)
 constexpr int kProducerWarpB = 2;       // B operand (bulk TMA)
 constexpr int kMmaWarp = 1;
-constexpr int kEpiWarp0 = 4;            // warps 4..11  (warp % 4 = TMEM lane quarter), 2 column halves
-constexpr int kEpiWarps = 8;
-constexpr int kAWarp0 = 12;             // warps 12..19 (warp % 4 = TMEM lane quarter), 2 sets
-constexpr int kUnpackWarp0 = 20;        // warps 20..27, 2 sets
+constexpr int kEpiWarp0 = 4;            // epilogue warps start here (warp % 4 = TMEM lane quarter)
 constexpr int kNumUnpackWarps = 4;      // per set
+constexpr int kAStageBytes = BM * BK;   // fused variant: int8 A operand stage in shared memory
 
-template <int CG>
+// CG = CTAs per tile (1 or 2).  FUSED = quantise-in-producer variant (a10): the eight A warps read
+// bf16 X, quantise with the per-token scale and write the int8 operand to SHARED memory (any
+// thread -> element mapping is allowed there; the Hadamard needs 16 lanes per 128 channels), and
+// the MMA takes both operands from shared memory (.ss form).
+template <int CG, bool FUSED>
 struct Cfg {
+  static constexpr int kEpiWarps = FUSED ? 4 : 8;           // x 32 rows; 2 column halves when 8
+  static constexpr int kSets = FUSED ? 1 : kSetsMax;
+  static constexpr int kAWarp0 = kEpiWarp0 + kEpiWarps;     // 8 A warps in both variants
+  static constexpr int kUnpackWarp0 = kAWarp0 + 8;
+  static constexpr int kThreads = 32 * (kUnpackWarp0 + kNumUnpackWarps * kSets);
   static constexpr int kBRows = BN / CG;                   // weight rows staged per CTA
   static constexpr int kPackedB = kBRows * BK / 2;
-  static constexpr int kPackedStage = kPackedA + kPackedB;  // multiple of 1024 (swizzle alignment)
+  static constexpr int kPackedAArea = FUSED ? 0 : kPackedA;
+  static constexpr int kPackedStage = kPackedAArea + kPackedB;   // unfused: multiple of 1024
   static constexpr int kUnpackedStage = kBRows * BK;
-  static constexpr int kFullCount = CG * (4 + kNumUnpackWarps);
+  static constexpr int kAOperand = FUSED ? kStages * kAStageBytes : 0;
+  static constexpr int kPFullCount = FUSED ? 1 : 2;
+  static constexpr int kPEmptyCount = FUSED ? kNumUnpackWarps : kNumUnpackWarps + 4;
+  static constexpr int kFullCount = CG * ((FUSED ? 8 : 4) + kNumUnpackWarps);
   static constexpr int kTemptyCount = CG * kEpiWarps;
   static constexpr int kPStages = CG == 2 ? kPStagesMax : 5;
-  static constexpr int kSmemBytes = 1024 + kStages * kUnpackedStage + kPStages * kPackedStage + 256;
+  static constexpr int kSmemBytes =
+      1024 + kAOperand + kStages * kUnpackedStage + kPStages * kPackedStage + 256;
   static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
 };
 
@@ -94,6 +106,15 @@ struct GemmParams {
   int32_t* acc_dump;        // optional [T, N]
   int T, N, K;
   int num_m, num_n, num_kb;
+  // fused variant only
+  const uint4* x;           // bf16 [T, ldx] viewed as 16-byte vectors
+  int64_t ldxv;             // ldx / 8
+  float gamma;
+  const float* sa;
+  const float* bvec;
+  int had_block;
+  float had_scale;
+  uint32_t* codes_dump;     // optional [T, K/8] words of 8 nibbles
 };
 
 __device__ __forceinline__ void advance(int& stage, uint32_t& phase, int n) {
@@ -154,18 +175,26 @@ __device__ __forceinline__ uint32_t dequant_bf16x2(int32_t a0, int32_t a1, float
 
 // ------------------------------------------------------------------------------ the kernel
 // CG = 1: one CTA per tile of 128 x BN;  CG = 2: a CTA pair per tile of 256 x BN.
-template <int CG>
-__global__ void __launch_bounds__(kNumThreads, 1)
+template <int CG, bool FUSED>
+__global__ void __launch_bounds__((Cfg<CG, FUSED>::kThreads), 1)
 w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
-  using C = Cfg<CG>;
+  using C = Cfg<CG, FUSED>;
+  constexpr int kEpiWarps = C::kEpiWarps;
+  constexpr int kSets = C::kSets;
+  constexpr int kAWarp0 = C::kAWarp0;
+  constexpr int kUnpackWarp0 = C::kUnpackWarp0;
   extern __shared__ uint8_t smem_raw[];
   // SWIZZLE_128B operands need 1024-byte alignment
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
-  const uint32_t unpacked0 = smem_base;
-  const uint32_t packed0 = smem_base + kStages * C::kUnpackedStage;
-  uint8_t* unpacked_ptr = smem;
-  uint8_t* packed_ptr = smem + kStages * C::kUnpackedStage;
+  // [ fused: int8 A stages | int8 B stages | packed ring | barriers ]
+  const uint32_t aop0 = smem_base;
+  uint8_t* aop_ptr = smem;
+  const uint32_t unpacked0 = smem_base + C::kAOperand;
+  const uint32_t packed0 = unpacked0 + kStages * C::kUnpackedStage;
+  uint8_t* unpacked_ptr = smem + C::kAOperand;
+  uint8_t* packed_ptr = unpacked_ptr + kStages * C::kUnpackedStage;
+  (void)aop0; (void)aop_ptr;
   Barriers* bars = reinterpret_cast<Barriers*>(packed_ptr + C::kPStages * C::kPackedStage);
 
   const int warp = threadIdx.x >> 5;
@@ -174,10 +203,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
   const bool leader = rank == 0;
 
   if (warp == kProducerWarp && lane == 0) {
-    ptx::prefetch_tensormap(&tmap_a);
+    if (!FUSED) ptx::prefetch_tensormap(&tmap_a);
     for (int i = 0; i < C::kPStages; ++i) {
-      ptx::mbar_init(ptx::smem_u32(&bars->pfull[i]), 2);
-      ptx::mbar_init(ptx::smem_u32(&bars->pempty[i]), kNumUnpackWarps + 4);
+      ptx::mbar_init(ptx::smem_u32(&bars->pfull[i]), C::kPFullCount);
+      ptx::mbar_init(ptx::smem_u32(&bars->pempty[i]), C::kPEmptyCount);
     }
     for (int i = 0; i < kStages; ++i) {
       ptx::mbar_init(ptx::smem_u32(&bars->full[i]), C::kFullCount);
@@ -203,7 +232,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
   const int first_tile = static_cast<int>(blockIdx.x) / CG;
   const int tile_step = static_cast<int>(gridDim.x) / CG;
 
-  if (warp == kProducerWarp || warp == kProducerWarpB) {
+  if ((warp == kProducerWarp && !FUSED) || warp == kProducerWarpB) {
     // ===================================================================== producers (TMA)
     // Two warps, one per operand: a single warp's wait + expect_tx + two copy issues per k-block
     // is a ~350 clk serial chain (measured with everything else stubbed out).
@@ -227,10 +256,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
             ptx::tma_load_2d(dst, &tmap_a, kb * (BK / 2), row0, full);
           } else {
             ptx::mbar_arrive_expect_tx(full, C::kPackedB);
-            ptx::bulk_load_1d(dst + kPackedA, g0 + static_cast<size_t>(kb) * kTileBytes,
+            ptx::bulk_load_1d(dst + C::kPackedAArea, g0 + static_cast<size_t>(kb) * kTileBytes,
                               kTileBytes, full);
             if (CG == 1) {
-              ptx::bulk_load_1d(dst + kPackedA + kTileBytes,
+              ptx::bulk_load_1d(dst + C::kPackedAArea + kTileBytes,
                                 g0 + static_cast<size_t>(p.num_kb + kb) * kTileBytes, kTileBytes,
                                 full);
             }
@@ -251,6 +280,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       int stage = 0, as = 0;
       uint32_t phase = 0, aphase = 0;
       const uint64_t desc0 = ptx::make_smem_desc_sw128(unpacked0);
+      const uint64_t adesc0 = ptx::make_smem_desc_sw128(aop0);
+      (void)adesc0;
       for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
         ptx::mbar_wait(ptx::smem_u32(&bars->tempty[as]), aphase ^ 1u);
         ptx::tcgen05_fence_after();
@@ -265,8 +296,14 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
 #pragma unroll
             for (int k = 0; k < BK / 32; ++k) {
               const uint32_t accum = (kb | k) != 0 ? 1u : 0u;
-              if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
-              else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+              if (FUSED) {
+                const uint64_t da = adesc0 + static_cast<uint64_t>(stage * (kAStageBytes >> 4)) + 2 * k;
+                if (CG == 2) ptx::mma_i8_ss_2cta(tmem_d, da, db + 2 * k, idesc, accum);
+                else ptx::mma_i8_ss(tmem_d, da, db + 2 * k, idesc, accum);
+              } else {
+                if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+                else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+              }
             }
             // frees the operand stage (A columns + B smem) in every CTA of the pair
             if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
@@ -301,7 +338,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           continue;
         }
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
-        const uint8_t* src = packed_ptr + ps * C::kPackedStage + kPackedA;
+        const uint8_t* src = packed_ptr + ps * C::kPackedStage + C::kPackedAArea;
         uint4 v[kTasks];
 #pragma unroll
         for (int i = 0; i < kTasks; ++i)
@@ -331,7 +368,92 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
         advance(us, uphase, kStages);
       }
     }
-  } else if (warp >= kAWarp0 && warp < kAWarp0 + 4 * kSets) {
+  } else if (FUSED && warp >= kAWarp0 && warp < kAWarp0 + 8) {
+    // ===================================================================== A: quantise in producer
+    // Eight warps x 32 lanes cover one 128-row x 128-channel k-block as 8 passes of 16 rows:
+    // lane = (row parity, vector v = lane & 15), so the 16 lanes of a half-warp hold the 128
+    // channels of one token (what the Hadamard's shuffle stages need) and a warp-wide load reads
+    // two rows x 256 contiguous bytes.  Same arithmetic (quant_math.cuh) and therefore the same
+    // codes as the stand-alone quantiser; the codes leave as 16 * q int8 in the even/odd order of
+    // the x16 expansion, straight into the SWIZZLE_128B operand stage.
+    const int aw = warp - kAWarp0;
+    const int v = lane & 15;
+    const int rbase = 2 * aw + (lane >> 4);               // rows rbase + 16 i, i = 0..7
+    const int r7 = rbase & 7;
+    const uint32_t full_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->full[0]), 0);
+    const uint32_t st_off = static_cast<uint32_t>((rbase >> 3) * 1024 + r7 * 128 + 4 * (v & 3));
+    const uint32_t ch_even = static_cast<uint32_t>(((2 * (v >> 2)) ^ r7) << 4);
+    const uint32_t ch_odd = static_cast<uint32_t>(((2 * (v >> 2) + 1) ^ r7) << 4);
+    // load cursor: one "half" (4 passes) ahead of the compute cursor
+    int l_tile = first_tile, l_kb = 0, l_half = 0;
+    auto load_half = [&](uint4 (&b)[4]) {
+      if (l_tile < num_tiles) {
+        const int row0 = (l_tile % p.num_m) * (BM * CG) + static_cast<int>(rank) * BM + rbase;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int row = row0 + 16 * (4 * l_half + i);
+          b[i] = row < p.T ? ptx::ldg_nc_stream(p.x + static_cast<int64_t>(row) * p.ldxv + l_kb * 16 + v)
+                           : make_uint4(0, 0, 0, 0);
+        }
+        if (++l_half == 2) {
+          l_half = 0;
+          if (++l_kb == p.num_kb) {
+            l_kb = 0;
+            l_tile += tile_step;
+          }
+        }
+      }
+    };
+    uint4 nxt[4];
+    load_half(nxt);
+    int us = 0;
+    uint32_t uphase = 0;
+    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
+      const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
+      const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM + rbase;
+      float inv[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int row = row0 + 16 * i;
+        inv[i] = row < p.T ? qm::reciprocal(p.scales[row]) : 0.0f;
+      }
+      const bool dump = p.codes_dump != nullptr && n_blk == 0;
+      for (int kb = 0; kb < p.num_kb; ++kb) {
+        float g[8], bb[8];
+        qm::load_gb(p.sa, p.bvec, p.gamma, kb * 16 + v, true, g, bb);
+        ptx::mbar_wait(ptx::smem_u32(&bars->empty[us]), uphase ^ 1u);
+        uint8_t* stage = aop_ptr + us * kAStageBytes + st_off;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          uint4 cur[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
+          load_half(nxt);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            float f[8];
+            qm::unpack8(cur[i], f);
+            if (p.had_block) qm::hadamard8(f, p.had_block, p.had_scale, lane);
+            uint32_t t[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) t[e] = qm::code_bits(qm::affine(g[e], f[e], bb[e]), inv[4 * h + i]);
+            const uint32_t pn = qm::pack_nibbles(t);
+            uint8_t* dst = stage + (4 * h + i) * 2048;      // 16 rows = two 1024-byte swizzle atoms
+            *reinterpret_cast<uint32_t*>(dst + ch_even) = (pn << 4) & 0xF0F0F0F0u;
+            *reinterpret_cast<uint32_t*>(dst + ch_odd) = pn & 0xF0F0F0F0u;
+            if (dump) {
+              const int row = row0 + 16 * (4 * h + i);
+              if (row < p.T) p.codes_dump[static_cast<int64_t>(row) * (p.K / 8) + kb * 16 + v] = pn;
+            }
+          }
+        }
+        ptx::fence_proxy_async_smem();      // generic-proxy writes -> visible to tcgen05.mma
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster(full_remote + us * 8);
+        advance(us, uphase, kStages);
+      }
+    }
+  } else if (!FUSED && warp >= kAWarp0 && warp < kAWarp0 + 8) {
     // ===================================================================== A: smem -> TMEM
     // thread = token row = TMEM lane.  The packed tile is [128 rows][64 B] with TMA's SWIZZLE_64B
     // (16-byte chunk index ^= (row >> 1) & 3), so the 32 lanes' 16-byte reads of one chunk column
@@ -481,13 +603,13 @@ EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-template <int CG>
+template <int CG, bool FUSED>
 cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sms,
                       cudaStream_t stream) {
-  using C = Cfg<CG>;
+  using C = Cfg<CG, FUSED>;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(w4a4_gemm_kernel<CG>,
+    cudaError_t e = cudaFuncSetAttribute(w4a4_gemm_kernel<CG, FUSED>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
     if (e != cudaSuccess) return e;
     attr_set = true;
@@ -497,7 +619,7 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sm
   const int groups = tiles < slots ? tiles : slots;
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(static_cast<unsigned>(groups * CG), 1, 1);
-  cfg.blockDim = dim3(kNumThreads, 1, 1);
+  cfg.blockDim = dim3(C::kThreads, 1, 1);
   cfg.dynamicSmemBytes = C::kSmemBytes;
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
@@ -507,23 +629,24 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sm
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG>, tmap_a, p);
+  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG, FUSED>, tmap_a, p);
 }
 
 }  // namespace
 
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
-  if (g.x != nullptr) return cudaErrorNotSupported;     // fused producer: see launch_w4a4_fused
+  const bool fused = g.x != nullptr;
+  if (fused && g.had_block > 128) return cudaErrorNotSupported;   // 16 lanes hold 128 channels
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
   const int cg = g.cta_group == 1 ? 1 : 2;
-  EncodeTiledFn encode = get_encode_fn();
-  if (encode == nullptr) return cudaErrorNotSupported;
 
-  // A operand: codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows, SWIZZLE_64B; rows
-  // beyond T are zero-filled by TMA, so a ragged last M tile needs no special case.
-  CUtensorMap tmap_a;
-  {
+  // A operand (unfused): codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows, SWIZZLE_64B;
+  // rows beyond T are zero-filled by TMA, so a ragged last M tile needs no special case.
+  CUtensorMap tmap_a{};
+  if (!fused) {
+    EncodeTiledFn encode = get_encode_fn();
+    if (encode == nullptr) return cudaErrorNotSupported;
     const cuuint64_t dims[2] = {static_cast<cuuint64_t>(g.K / 2), static_cast<cuuint64_t>(g.T)};
     const cuuint64_t strides[1] = {static_cast<cuuint64_t>(g.K / 2)};
     const cuuint32_t box[2] = {static_cast<cuuint32_t>(BK / 2), static_cast<cuuint32_t>(BM)};
@@ -535,7 +658,7 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
   }
 
-  GemmParams p;
+  GemmParams p{};
   p.tiles = base + h.off_tiles;
   p.sw = reinterpret_cast<const float*>(base + h.off_sw);
   p.fb = reinterpret_cast<const float*>(base + h.off_fb);
@@ -549,8 +672,20 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   p.num_m = (g.T + BM * cg - 1) / (BM * cg);
   p.num_n = h.Npad / BN;
   p.num_kb = g.K / BK;
-  return cg == 2 ? launch_cg<2>(tmap_a, p, g.num_sms, g.stream)
-                 : launch_cg<1>(tmap_a, p, g.num_sms, g.stream);
+  if (fused) {
+    p.x = static_cast<const uint4*>(g.x);
+    p.ldxv = g.ldx / 8;
+    p.gamma = g.gamma;
+    p.sa = g.sa;
+    p.bvec = g.b;
+    p.had_block = g.had_block;
+    p.had_scale = g.had_scale;
+    p.codes_dump = reinterpret_cast<uint32_t*>(g.codes_dump);
+    return cg == 2 ? launch_cg<2, true>(tmap_a, p, g.num_sms, g.stream)
+                   : launch_cg<1, true>(tmap_a, p, g.num_sms, g.stream);
+  }
+  return cg == 2 ? launch_cg<2, false>(tmap_a, p, g.num_sms, g.stream)
+                 : launch_cg<1, false>(tmap_a, p, g.num_sms, g.stream);
 }
 
 }  // namespace baseq

@@ -215,3 +215,66 @@ def test_abi_error_codes():
     with pytest.raises(bq.BaseqError) as e:
         bq.quantize_act(torch.zeros((0, 256), dtype=torch.bfloat16, device="cuda"), bq.ActParams(0.9))
     assert e.value.status == 2
+
+
+# ------------------------------------------------------------------------------- fused variant (a10)
+def run_fused(x_bits, W, alpha, gamma, b, had_block=0, sa=None):
+    """baseq_linear_fused vs the oracle: scales, producer codes, int32 accumulators, bf16 Y."""
+    N, K = W["N"], W["K"]
+    T = x_bits.shape[0]
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None if b is None else dev(b),
+                         None if W["layer_bias"] is None else dev(W["layer_bias"]))
+    params = bq.ActParams(alpha, gamma, None if sa is None else dev(sa),
+                          None if b is None else dev(b), had_block)
+    codes = torch.zeros((T, K // 2), dtype=torch.uint8, device="cuda")
+    acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
+    y, scales = bq.linear_fused(bf16_dev(x_bits), params, pw, codes_dump=codes, acc_dump=acc)
+    y2, _ = bq.linear_fused(bf16_dev(x_bits), params, pw)          # timed configuration: no dumps
+    torch.cuda.synchronize()
+    assert torch.equal(y.view(torch.int16), y2.view(torch.int16))
+    ref = oracle.linear(x_bits, W["w_nibbles"], W["w_scale"], fb, alpha, gamma, sa, b, had_block)
+    assert np.array_equal(scales.cpu().numpy().view(np.uint32), ref["scales"].view(np.uint32))
+    assert np.array_equal(codes.cpu().numpy(), ref["codes"])
+    assert np.array_equal(acc.cpu().numpy(), ref["acc"])
+    assert np.array_equal(bits_host(y), ref["y"])
+
+
+def _rand_w(rng, N, K, bias=True):
+    q = rng.integers(-8, 8, size=(N, K)).astype(np.int8).astype(np.uint8) & 0xF
+    return {"N": N, "K": K, "w_nibbles": np.ascontiguousarray(q[:, 0::2] | (q[:, 1::2] << 4)),
+            "w_scale": (0.002 + 0.004 * rng.random(N)).astype(np.float32),
+            "layer_bias": rng.standard_normal(N).astype(np.float32) if bias else None}
+
+
+def test_fused_config1():
+    L = make_layer("c1", "linear")
+    sp = L["spec"]
+    run_fused(L["x"], L, sp.alpha, sp.gamma, L["b"])
+
+
+@pytest.mark.parametrize("T,K,N,B", [(1, 128, 8, 0), (130, 384, 264, 0), (257, 1024, 520, 128),
+                                     (300, 2048, 200, 16), (40, 4096, 192, 128)])
+def test_fused_ragged_and_hadamard(T, K, N, B):
+    rng = np.random.default_rng(T + 3 * K + 5 * N + B)
+    x = rand_x(rng, T, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    run_fused(x, _rand_w(rng, N, K), 0.9, 1.05, b, had_block=B)
+
+
+def test_fused_per_channel_sa_and_no_bias():
+    rng = np.random.default_rng(99)
+    T, K, N = 70, 512, 136
+    x = rand_x(rng, T, K)
+    sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+    run_fused(x, _rand_w(rng, N, K, bias=False), 1.0, 1.0, None, sa=sa)
+
+
+def test_fused_rejects_hadamard_256():
+    x = torch.zeros((4, 512), dtype=torch.bfloat16, device="cuda")
+    rng = np.random.default_rng(1)
+    W = _rand_w(rng, 8, 512)
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]))
+    with pytest.raises(bq.BaseqError) as e:
+        bq.linear_fused(x, bq.ActParams(0.9, had_block=256), pw)
+    assert e.value.status == 6
