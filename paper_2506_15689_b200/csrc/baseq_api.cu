@@ -11,6 +11,8 @@ namespace {
 
 using namespace baseq;
 
+int quant_blocks_per_sm();
+
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 struct DeviceInfo {
@@ -78,7 +80,19 @@ QuantLaunch make_quant(const void* x, int64_t ldx, int T, int K, const baseq_act
   q.stream = static_cast<cudaStream_t>(stream);
   q.tpr_log2 = 0;
   q.tpr_log2_override = 0;
+  q.num_sms = 148;          // overwritten by the callers from the device query
+  q.blocks_per_sm = quant_blocks_per_sm();
   return q;
+}
+
+// Tuning hook for profiling runs only: resident quantiser blocks per SM (default 2).
+int quant_blocks_per_sm() {
+  static int v = 0;
+  if (v == 0) {
+    const char* e = std::getenv("BASEQ_QUANT_BLOCKS_PER_SM");
+    v = (e != nullptr && e[0] >= '1' && e[0] <= '8') ? e[0] - '0' : 2;
+  }
+  return v;
 }
 
 // Tuning hook for profiling runs only: BASEQ_GEMM_CTA_GROUP=1 selects the single-CTA tiles.
@@ -153,10 +167,12 @@ baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int T, int K,
   if (st != BASEQ_OK) return st;
   if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4)) return BASEQ_ERR_ALIGN;
   if (ldx < K || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;
-  st = device_check(nullptr);
+  int sms = 0;
+  st = device_check(&sms);
   if (st != BASEQ_OK) return st;
-  const cudaError_t e =
-      launch_quantize_act(make_quant(x_bf16, ldx, T, K, p, codes, scales, stream), true);
+  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
+  q.num_sms = sms;
+  const cudaError_t e = launch_quantize_act(q, true);
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
 }
 
@@ -219,8 +235,9 @@ baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
   st = device_check(&sms);
   if (st != BASEQ_OK) return st;
   // pass 1: per-token absmax -> scales (reads X once, writes T floats)
-  cudaError_t e = launch_quantize_act(make_quant(x_bf16, ldx, T, K, p, nullptr, scales_out, stream),
-                                      false);
+  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, nullptr, scales_out, stream);
+  q.num_sms = sms;
+  cudaError_t e = launch_quantize_act(q, false);
   if (e != cudaSuccess) return BASEQ_ERR_CUDA;
   // pass 2: GEMM with the quantise-in-producer variant
   GemmLaunch g{};

@@ -59,6 +59,8 @@ struct QuantLaunch {
   cudaStream_t stream;
   int tpr_log2;            // filled by the launcher
   int tpr_log2_override;   // 0 = heuristic (tuning hook for profiling runs)
+  int num_sms;             // persistent grid = num_sms * blocks_per_sm
+  int blocks_per_sm;
 };
 int quant_max_k();
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes);
