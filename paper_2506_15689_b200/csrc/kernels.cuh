@@ -64,6 +64,9 @@ struct QuantLaunch {
 };
 int quant_max_k();
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes);
+// long rows (K >= 4096): bulk-TMA ring variant of the same contract (quantize_ring.cu)
+bool quantize_ring_supported(int K);
+cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes);
 
 // ------------------------------------------------------------------ weight packer
 cudaError_t launch_pack_weights(const uint8_t* w_nibbles, const float* w_scale, const float* b,

@@ -108,5 +108,27 @@ __device__ __forceinline__ uint32_t pack_nibbles(const uint32_t (&t)[8]) {
   return __byte_perm(lo, hi, 0x5410);                // lo.b0 lo.b1 hi.b0 hi.b1
 }
 
+
+// Q6 + Q7 for 8 channels at once.  Only the lower clamp is done in floating point; the magic add
+// rounds (RNE), an integer subtract recovers the signed code and cvt.pack.sat.s4.s32 saturates to
+// [-8, 7] and packs two codes per instruction:  d = (c << 8) | (sat(a) << 4) | (sat(b) & 15).
+// For r >= 2^22 the magic add is no longer exact but stays a large positive integer, which
+// saturates to 7 as required.
+__device__ __forceinline__ int32_t code_int(float u, float inv) {
+  const float r = fmaxf(__fmul_rn(u, inv), -8.0f);
+  return static_cast<int32_t>(__float_as_uint(__fadd_rn(r, 12582912.0f))) - 0x4B400000;
+}
+__device__ __forceinline__ uint32_t pack2_sat(int32_t hi, int32_t lo, uint32_t prev) {
+  uint32_t d;
+  asm("cvt.pack.sat.s4.s32.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(hi), "r"(lo), "r"(prev));
+  return d;
+}
+__device__ __forceinline__ uint32_t quantize_pack8(const float (&u)[8], float inv) {
+  uint32_t w = pack2_sat(code_int(u[7], inv), code_int(u[6], inv), 0u);
+  w = pack2_sat(code_int(u[5], inv), code_int(u[4], inv), w);
+  w = pack2_sat(code_int(u[3], inv), code_int(u[2], inv), w);
+  return pack2_sat(code_int(u[1], inv), code_int(u[0], inv), w);
+}
+
 }  // namespace qm
 }  // namespace baseq

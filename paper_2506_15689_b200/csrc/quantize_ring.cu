@@ -1,0 +1,284 @@
+// Activation quantiser for long rows (K >= 4096): the same arithmetic contract as
+// quantize_act.cu (quant_math.cuh), fed by a bulk-TMA ring.
+//
+// Why: the register-resident row kernel keeps only its own loads in flight (32-64 KB per SM) and
+// measured 2.5-3.0 TB/s (profiles/).  Here one producer lane streams whole token rows
+// (row-contiguous cp.async.bulk copies, completion on an mbarrier) into a ring of shared-memory
+// stages that fills whatever the 227 KB allow -- 150-200 KB of loads in flight per SM, no
+// registers involved -- and 16 consumer warps (512 threads = one row wide, thread r owns the
+// 16-byte vectors r, r + 512, ...) read each stage once from shared memory, conflict-free.
+//
+// Per stage of RL rows: pass 1 (u = g h - b, absmax) -> the stage is released to the producer ->
+// block reduction (partials in smem, one designated warp per row finishes the max and computes
+// s_t and 1 / s_t once) -> pass 2 from registers (round, clamp, pack, store).
+#include "kernels.cuh"
+#include "ptx.cuh"
+#include "quant_math.cuh"
+
+namespace baseq {
+namespace {
+
+constexpr int kConsumers = 512;                 // threads per row
+constexpr int kConsumerWarps = kConsumers / 32;
+constexpr int kRingThreads = kConsumers + 32;   // + the producer warp
+constexpr int kMaxStages = 8;
+constexpr int kRingSmemBudget = 220 * 1024;
+
+struct RingParams {
+  const uint8_t* x;        // bf16 rows
+  int64_t row_bytes_stride;
+  int T, K, nvec;
+  float alpha, gamma;
+  const float* sa;
+  const float* bvec;
+  int had_block;
+  float had_scale;
+  uint32_t* codes;
+  float* scales;
+  int stages;
+  int stage_bytes;
+};
+
+__device__ __forceinline__ void named_barrier_sync(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+template <int V, int RL, bool HAD, bool WRITE_CODES, bool RAGGED>
+__global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const RingParams p) {
+  extern __shared__ __align__(128) uint8_t ring[];
+  __shared__ uint64_t full[kMaxStages], empty[kMaxStages];
+  __shared__ float s_part[2][RL][kConsumerWarps];
+  __shared__ float2 s_scale[2][RL];
+
+  const int tid = threadIdx.x;
+  const int warp = tid >> 5, lane = tid & 31;
+  const int num_groups = (p.T + RL - 1) / RL;     // one group = RL rows = one stage
+
+  if (tid == 0) {
+    for (int s = 0; s < p.stages; ++s) {
+      ptx::mbar_init(ptx::smem_u32(&full[s]), 1);
+      ptx::mbar_init(ptx::smem_u32(&empty[s]), kConsumerWarps);
+    }
+    ptx::fence_barrier_init();
+  }
+  __syncthreads();
+
+  if (warp == kConsumerWarps) {
+    // ===================================================================== producer
+    if (lane == 0) {
+      int s = 0;
+      uint32_t ph = 0;
+      const uint32_t row_bytes = static_cast<uint32_t>(p.K) * 2u;
+      for (int g = blockIdx.x; g < num_groups; g += gridDim.x) {
+        ptx::mbar_wait(ptx::smem_u32(&empty[s]), ph ^ 1u);
+        const int row0 = g * RL;
+        const int rows = (p.T - row0) < RL ? (p.T - row0) : RL;
+        const uint32_t bar = ptx::smem_u32(&full[s]);
+        ptx::mbar_arrive_expect_tx(bar, row_bytes * rows);
+        const uint32_t dst = ptx::smem_u32(ring) + s * p.stage_bytes;
+        for (int j = 0; j < rows; ++j) {
+          ptx::bulk_load_1d(dst + j * row_bytes, p.x + static_cast<int64_t>(row0 + j) * p.row_bytes_stride,
+                            row_bytes, bar);
+        }
+        if (++s == p.stages) { s = 0; ph ^= 1u; }
+      }
+    }
+    return;
+  }
+
+  // ======================================================================= consumers
+  const int r = tid;                               // vector r + i * 512 of every row
+  constexpr bool kBiasInRegs = V <= 4;
+  float bb[kBiasInRegs ? V : 1][8];
+  if (kBiasInRegs) {
+#pragma unroll
+    for (int i = 0; i < V; ++i) {
+      const int idx = r + i * kConsumers;
+      float g_unused[8];
+      qm::load_gb(nullptr, p.bvec, p.gamma, idx, !RAGGED || idx < p.nvec, g_unused,
+                  bb[kBiasInRegs ? i : 0]);
+    }
+  }
+
+  int s = 0, parity = 0;
+  uint32_t ph = 0;
+  for (int g = blockIdx.x; g < num_groups; g += gridDim.x, parity ^= 1) {
+    const int row0 = g * RL;
+    ptx::mbar_wait(ptx::smem_u32(&full[s]), ph);
+    const uint8_t* stage = ring + s * p.stage_bytes;
+
+    // ---- pass 1: smem -> registers, Hadamard, u = g*h - b, absmax
+    float u[RL][V][8];
+    float m[RL];
+#pragma unroll
+    for (int j = 0; j < RL; ++j) {
+      m[j] = 0.0f;
+#pragma unroll
+      for (int i = 0; i < V; ++i) {
+        const int idx = r + i * kConsumers;
+        const bool ok = !RAGGED || idx < p.nvec;
+        uint4 xv = make_uint4(0, 0, 0, 0);
+        if (ok) xv = *reinterpret_cast<const uint4*>(stage + static_cast<size_t>(j) * p.K * 2 + idx * 16);
+        float f[8];
+        qm::unpack8(xv, f);
+        if (HAD) qm::hadamard8(f, p.had_block, p.had_scale, lane);
+        float gl[8], bl[8];
+        if (p.sa != nullptr || !kBiasInRegs) {
+          qm::load_gb(p.sa, kBiasInRegs ? nullptr : p.bvec, p.gamma, idx, ok, gl, bl);
+        }
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          const float gg = p.sa != nullptr ? gl[e] : p.gamma;
+          const float bv = kBiasInRegs ? bb[kBiasInRegs ? i : 0][e] : bl[e];
+          u[j][i][e] = qm::affine(gg, f[e], bv);
+          m[j] = fmaxf(m[j], fabsf(u[j][i][e]));
+        }
+      }
+    }
+    // every lane's shared-memory reads have returned (their values fed the max): release the stage
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&empty[s]));
+    if (++s == p.stages) { s = 0; ph ^= 1u; }
+
+    // ---- block reduction: warp shuffle -> partials -> one warp per row finishes.
+    // RL row maxima are reduced together: each xor step that halves the live values costs one
+    // shuffle per surviving value (6 shuffles for 4 rows instead of 20).
+    if (RL == 4) {
+      const bool up16 = (lane & 16) != 0, up8 = (lane & 8) != 0;
+      float s0 = up16 ? m[0] : m[2], s1 = up16 ? m[1] : m[3];      // what the partner keeps
+      float k0 = up16 ? m[2] : m[0], k1 = up16 ? m[3] : m[1];
+      k0 = fmaxf(k0, __shfl_xor_sync(0xffffffffu, s0, 16));
+      k1 = fmaxf(k1, __shfl_xor_sync(0xffffffffu, s1, 16));
+      const float snd = up8 ? k0 : k1;
+      float c = up8 ? k1 : k0;
+      c = fmaxf(c, __shfl_xor_sync(0xffffffffu, snd, 8));
+#pragma unroll
+      for (int o = 4; o > 0; o >>= 1) c = fmaxf(c, __shfl_xor_sync(0xffffffffu, c, o));
+      // lane 0, 8, 16, 24 hold rows 0, 1, 2, 3
+      if ((lane & 7) == 0) s_part[parity][lane >> 3][warp] = c;
+    } else if (RL == 2) {
+      const bool up16 = (lane & 16) != 0;
+      const float snd = up16 ? m[0] : m[1 % RL];
+      float c = up16 ? m[1 % RL] : m[0];
+      c = fmaxf(c, __shfl_xor_sync(0xffffffffu, snd, 16));
+#pragma unroll
+      for (int o = 8; o > 0; o >>= 1) c = fmaxf(c, __shfl_xor_sync(0xffffffffu, c, o));
+      if ((lane & 15) == 0) s_part[parity][(lane >> 4) % RL][warp] = c;
+    } else {
+#pragma unroll
+      for (int j = 0; j < RL; ++j) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m[j] = fmaxf(m[j], __shfl_xor_sync(0xffffffffu, m[j], o));
+        if (lane == 0) s_part[parity][j][warp] = m[j];
+      }
+    }
+    named_barrier_sync(1, kConsumers);
+    if (warp < RL) {
+      float mm = lane < kConsumerWarps ? s_part[parity][warp][lane] : 0.0f;
+#pragma unroll
+      for (int o = 8; o > 0; o >>= 1) mm = fmaxf(mm, __shfl_xor_sync(0xffffffffu, mm, o));
+      if (lane == 0) {
+        const float st = qm::step_size(p.alpha, mm);
+        s_scale[parity][warp] = make_float2(st, qm::reciprocal(st));
+        if (row0 + warp < p.T) p.scales[row0 + warp] = st;
+      }
+    }
+    named_barrier_sync(2, kConsumers);
+
+    // ---- pass 2: round, clamp, pack, store
+    if (WRITE_CODES) {
+#pragma unroll
+      for (int j = 0; j < RL; ++j) {
+        const float inv = s_scale[parity][j].y;
+        if (row0 + j < p.T) {
+          uint32_t* crow = p.codes + static_cast<int64_t>(row0 + j) * p.nvec;
+#pragma unroll
+          for (int i = 0; i < V; ++i) {
+            const int idx = r + i * kConsumers;
+            const uint32_t w = qm::quantize_pack8(u[j][i], inv);
+            if (!RAGGED || idx < p.nvec) crow[idx] = w;
+          }
+        }
+      }
+    }
+  }
+}
+
+template <int V, int RL, bool HAD, bool WC, bool RAGGED>
+cudaError_t launch_ring_r(const QuantLaunch& q) {
+  RingParams p{};
+  p.x = static_cast<const uint8_t*>(q.x);
+  p.row_bytes_stride = q.ldx * 2;
+  p.T = q.T;
+  p.K = q.K;
+  p.nvec = q.K / 8;
+  p.alpha = q.alpha;
+  p.gamma = q.gamma;
+  p.sa = q.sa;
+  p.bvec = q.b;
+  p.had_block = q.had_block;
+  p.had_scale = q.had_scale;
+  p.codes = reinterpret_cast<uint32_t*>(q.codes);
+  p.scales = q.scales;
+  p.stage_bytes = RL * q.K * 2;
+  int stages = kRingSmemBudget / p.stage_bytes;
+  p.stages = stages > kMaxStages ? kMaxStages : stages;
+  if (p.stages < 2) return cudaErrorInvalidValue;
+  const int smem = p.stages * p.stage_bytes;
+  static int attr_smem = 0;
+  if (smem > attr_smem) {
+    cudaError_t e = cudaFuncSetAttribute(quantize_ring_kernel<V, RL, HAD, WC, RAGGED>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    attr_smem = smem;
+  }
+  const int groups = (q.T + RL - 1) / RL;
+  const int blocks = groups < q.num_sms ? groups : q.num_sms;
+  quantize_ring_kernel<V, RL, HAD, WC, RAGGED><<<blocks, kRingThreads, smem, q.stream>>>(p);
+  return cudaGetLastError();
+}
+
+template <int V, int RL, bool HAD, bool WC>
+cudaError_t launch_ring_t(const QuantLaunch& q) {
+  return (q.K / 8) % kConsumers != 0 ? launch_ring_r<V, RL, HAD, WC, true>(q)
+                                     : launch_ring_r<V, RL, HAD, WC, false>(q);
+}
+
+template <bool HAD, bool WC>
+cudaError_t launch_ring_hw(const QuantLaunch& q, int V, int RL) {
+  // reachable (V, RL): RL = 4 for K <= 5120 (V <= 2), RL = 2 for K <= 10240 (V = 2, 3), else RL = 1
+  if (RL == 4) {
+    if (V == 1) return launch_ring_t<1, 4, HAD, WC>(q);
+    if (V == 2) return launch_ring_t<2, 4, HAD, WC>(q);
+  } else if (RL == 2) {
+    if (V == 2) return launch_ring_t<2, 2, HAD, WC>(q);
+    if (V == 3) return launch_ring_t<3, 2, HAD, WC>(q);
+  } else {
+    switch (V) {
+      case 3: return launch_ring_t<3, 1, HAD, WC>(q);
+      case 4: return launch_ring_t<4, 1, HAD, WC>(q);
+      case 5: return launch_ring_t<5, 1, HAD, WC>(q);
+      case 6: return launch_ring_t<6, 1, HAD, WC>(q);
+      case 7: return launch_ring_t<7, 1, HAD, WC>(q);
+      case 8: return launch_ring_t<8, 1, HAD, WC>(q);
+      default: break;
+    }
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+bool quantize_ring_supported(int K) { return K >= 4096 && K <= 32768; }
+
+cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes) {
+  const int nvec = q.K / 8;
+  const int V = (nvec + kConsumers - 1) / kConsumers;
+  const int RL = q.K <= 5120 ? 4 : (q.K <= 10240 ? 2 : 1);
+  if (q.had_block) {
+    return write_codes ? launch_ring_hw<true, true>(q, V, RL) : launch_ring_hw<true, false>(q, V, RL);
+  }
+  return write_codes ? launch_ring_hw<false, true>(q, V, RL) : launch_ring_hw<false, false>(q, V, RL);
+}
+
+}  // namespace baseq
