@@ -288,12 +288,15 @@ def run_gpu(args):
                 "frac_of_nominal_4500": tops / 4500.0,
                 "avg_launch_ms": gemm_ms / n_gemm, "share_of_step": gemm_ms / per_kernel.sum()}
     qgbs = quant_bytes / (quant_ms * 1e-3) / 1e9
-    roofline_q = {"bound": "hbm", "kernel": "quantize_act_kernel", "achieved": qgbs,
+    roofline_q = {"bound": "hbm", "kernel": "quantize_ring_kernel", "achieved": qgbs,
                   "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": qgbs / peaks["hbm_gbs"],
                   "frac_of_nominal_8000": qgbs / 8000.0, "share_of_step": quant_ms / per_kernel.sum()}
     per_layer = [{"kernel": kd[0], "name": kd[1], "ms": float(per_kernel[i]),
                   "rate": float(kd[2] / (per_kernel[i] * 1e-3) / (1e12 if kd[0] == "gemm" else 1e9)),
                   "rate_unit": "TOP/s" if kd[0] == "gemm" else "GB/s"} for i, kd in enumerate(kernels)]
+
+    # ---- the fused variant (a10) on the same layers, reported beside the two-kernel path
+    fused = run_fused(args, bq, torch, plan, acts, layers, T)
 
     # ---- end-to-end: HOST buffers through baseq_linear_host (H2D of X and D2H of Y timed)
     e2e = run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank)
@@ -304,13 +307,38 @@ def run_gpu(args):
             "dtype": "int4xint4->int32 (tcgen05 kind::i8); fp32 quantizer; bf16 out",
             "data": "synthetic", "config": workload_config(config), "clocks": clocks,
             "e2e": e2e, "gpu_launches": nk * args.steps, "roofline": roofline,
-            "roofline_quantizer": roofline_q, "kernels": per_layer}
+            "roofline_quantizer": roofline_q, "kernels": per_layer, "fused_variant": fused}
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(config, data, plan, layers, torch)
     if rank == 0:
         print(json.dumps(line))
     if ws > 1:
         dist.destroy_process_group()
+
+
+def run_fused(args, bq, torch, plan, acts, layers, T):
+    """baseq_linear_fused (absmax pre-pass + quantise-in-producer GEMM) per layer, same inputs."""
+    steps = max(3, min(args.steps, 20))
+    out = []
+    for act, specs in plan:
+        a = acts[act]
+        for sp in specs:
+            L = layers[sp.name]
+            y = torch.empty_like(L["y"])
+            for _ in range(3):
+                bq.linear_fused(a["x"], a["params"], L["pw"], y, scales=a["scales"])
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                bq.linear_fused(a["x"], a["params"], L["pw"], y, scales=a["scales"])
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            out.append({"name": sp.name, "ms": ms, "tokens_per_s": T / (ms * 1e-3),
+                        "same_bits_as_two_kernel_path": bool(torch.equal(
+                            y.view(torch.int16), L["y"].view(torch.int16)))})
+    return out
 
 
 def run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank):

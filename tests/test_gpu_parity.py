@@ -278,3 +278,52 @@ def test_fused_rejects_hadamard_256():
     with pytest.raises(bq.BaseqError) as e:
         bq.linear_fused(x, bq.ActParams(0.9, had_block=256), pw)
     assert e.value.status == 6
+
+
+# ------------------------------------------------------------------------------- full BASELINE sizes
+# Launch configuration = the one bench.py times (full T, N, K; no dumps for the timed output); the
+# oracle recomputes SAMPLED token rows one by one (first / middle / last tiles and the ragged end).
+def check_full(config, name, nrows=12, fused=False):
+    L = make_layer(config, name)
+    sp = L["spec"]
+    T = sp.T
+    rows = np.unique(np.r_[0:3, T // 2 - 1:T // 2 + 2, 255:258, T - 3:T])[:nrows + 3]
+    fb = oracle.fused_bias(L["w_nibbles"], L["w_scale"], L["b"], L["layer_bias"])
+    pw = bq.pack_weights(dev(L["w_nibbles"]), dev(L["w_scale"]), dev(L["b"]),
+                         None if L["layer_bias"] is None else dev(L["layer_bias"]))
+    params = bq.ActParams(sp.alpha, sp.gamma, None, dev(L["b"]), sp.had_block)
+    xd = bf16_dev(L["x"])
+    if fused:
+        y, scales = bq.linear_fused(xd, params, pw)
+        codes = None
+    else:
+        codes, scales = bq.quantize_act(xd, params)
+        y = bq.w4a4_gemm(codes, scales, pw)
+    torch.cuda.synchronize()
+    assert np.array_equal(pw.fused_bias.cpu().numpy().view(np.uint32), fb.view(np.uint32))
+    ref = oracle.linear(np.ascontiguousarray(L["x"][rows]), L["w_nibbles"], L["w_scale"], fb,
+                        sp.alpha, sp.gamma, None, L["b"], sp.had_block)
+    assert np.array_equal(scales.cpu().numpy()[rows].view(np.uint32), ref["scales"].view(np.uint32))
+    if codes is not None:
+        assert np.array_equal(codes[torch.from_numpy(rows).cuda()].cpu().numpy(), ref["codes"])
+    gy = bits_host(y[torch.from_numpy(rows).cuda()])
+    nbad = int((gy != ref["y"]).sum())
+    assert nbad == 0, "%s/%s: %d of %d sampled bf16 outputs differ" % (config, name, nbad, gy.size)
+
+
+@pytest.mark.parametrize("config,name", [("c2", "qkvo"), ("c3", "up"), ("c3", "down"), ("c4", "k"),
+                                         ("c4", "o"), ("c4", "up"), ("c4", "down"), ("c5", "down")])
+def test_full_size_sampled_rows(config, name):
+    check_full(config, name)
+
+
+@pytest.mark.parametrize("config,name", [("c3", "down"), ("c4", "k")])
+def test_full_size_fused_sampled_rows(config, name):
+    check_full(config, name, fused=True)
+
+
+def test_config5_fused_hadamard_small_T():
+    A = make_activations("c5", "x_down", T=70)
+    rng = np.random.default_rng(55)
+    W = _rand_w(rng, 200, 28672, bias=False)
+    run_fused(A["x"], W, 0.9, 1.0, A["b"], had_block=128)
