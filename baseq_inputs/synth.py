@@ -32,8 +32,8 @@ class LayerSpec:
 # gamma for config 3 comes from the 1-D grid stand-in of reading C-12; the values are
 # written by oracle/calibrate_gamma.py (calls only oracle/) into tests/golden/c3_gamma.json
 # and copied here by hand (a stored constant, not computed at run time).
-C3_GAMMA_MLP = 1.03
-C3_GAMMA_DOWN = 1.10
+C3_GAMMA_MLP = 1.00
+C3_GAMMA_DOWN = 1.00
 
 CONFIGS = {
     "c1": [LayerSpec("c1", "linear", 16, 256, 256, "x", 0.9, 1.05, 0, 0, True)],
