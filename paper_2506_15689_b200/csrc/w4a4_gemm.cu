@@ -153,24 +153,26 @@ __device__ __noinline__ uint32_t dequant_f64(int32_t acc, float st, float sw, fl
   const double yd = __fma_rn(pd, static_cast<double>(acc), static_cast<double>(fb));
   return bf16_from_double_rne(yd);
 }
-__device__ __forceinline__ uint32_t dequant_bf16(int32_t acc, float st, float sw, float fb) {
-  // exact int -> float without the quarter-rate I2F: |acc| <= 64 K < 2^22
-  const float accf = __fsub_rn(__int_as_float(0x4B400000 + acc), 12582912.0f);
-  const float t = __fmul_rn(st, accf);
+// `raw` is the TMEM accumulator 256 * acc (|acc| < 2^22, so raw has at most 22 significant bits
+// and converts to fp32 exactly) and st256 = s_t * 2^-8 (exact): st256 * float(raw) is the same
+// real number as s_t * acc and rounds to the same t.
+__device__ __forceinline__ uint32_t dequant_bf16(int32_t raw, float st256, float st, float sw,
+                                                 float fb) {
+  const float t = __fmul_rn(st256, __int2float_rn(raw));
   const float p = __fmul_rn(t, sw);
   const float y = __fmaf_rn(t, sw, fb);
-  const float e = __fmul_rn(__fadd_rn(fabsf(p), fabsf(y)), 1.1920928955078125e-07f);   // 2^-23
-  const float lo = __fsub_rn(y, e);
-  const float hi = __fadd_rn(y, e);
+  const float s = __fadd_rn(fabsf(p), fabsf(y));
+  const float hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);     // y + 2^-23 (|p| + |y|)
+  const float lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
   uint32_t pk;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));   // hi -> upper half
   const uint32_t a = pk & 0xFFFFu, b = pk >> 16;
   if (a == b && fabsf(y) > 1e-30f) return a;
-  return dequant_f64(acc, st, sw, fb);
+  return dequant_f64(raw >> 8, st, sw, fb);
 }
-__device__ __forceinline__ uint32_t dequant_bf16x2(int32_t a0, int32_t a1, float st, float2 sw,
-                                                   float2 fb) {
-  return dequant_bf16(a0, st, sw.x, fb.x) | (dequant_bf16(a1, st, sw.y, fb.y) << 16);
+__device__ __forceinline__ uint32_t dequant_bf16x2(int32_t r0, int32_t r1, float st256, float st,
+                                                   float2 sw, float2 fb) {
+  return dequant_bf16(r0, st256, st, sw.x, fb.x) | (dequant_bf16(r1, st256, st, sw.y, fb.y) << 16);
 }
 
 // ------------------------------------------------------------------------------ the kernel
@@ -518,6 +520,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       const int row = m_blk * (BM * CG) + static_cast<int>(rank) * BM + q * 32 + lane;
       const bool row_ok = row < p.T;
       const float st = row_ok ? p.scales[row] : 0.0f;
+      const float st256 = __fmul_rn(st, 0.00390625f);
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
       ptx::tcgen05_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN +
@@ -534,13 +537,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
 #pragma unroll
         for (int j = 0; j < 16; j += 2) {
           const int n = n0 + c0 + j;
-          const int32_t a0 = static_cast<int32_t>(r[j]) >> 8;       // raw = 256 * acc
-          const int32_t a1 = static_cast<int32_t>(r[j + 1]) >> 8;
-          r[j] = static_cast<uint32_t>(a0);
-          r[j + 1] = static_cast<uint32_t>(a1);
           const float2 sw = __ldg(reinterpret_cast<const float2*>(p.sw + n));
           const float2 fb = __ldg(reinterpret_cast<const float2*>(p.fb + n));
-          out[j >> 1] = dequant_bf16x2(a0, a1, st, sw, fb);
+          out[j >> 1] = dequant_bf16x2(static_cast<int32_t>(r[j]), static_cast<int32_t>(r[j + 1]),
+                                       st256, st, sw, fb);
         }
         if (row_ok) {
 #pragma unroll
@@ -551,9 +551,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
                   make_uint4(out[4 * g], out[4 * g + 1], out[4 * g + 2], out[4 * g + 3]);
               if (p.acc_dump != nullptr) {
                 int32_t* d = p.acc_dump + static_cast<int64_t>(row) * p.N + n;
-                *reinterpret_cast<uint4*>(d) = make_uint4(r[8 * g], r[8 * g + 1], r[8 * g + 2], r[8 * g + 3]);
-                *reinterpret_cast<uint4*>(d + 4) =
-                    make_uint4(r[8 * g + 4], r[8 * g + 5], r[8 * g + 6], r[8 * g + 7]);
+#pragma unroll
+                for (int e = 0; e < 8; ++e) d[e] = static_cast<int32_t>(r[8 * g + e]) >> 8;   // raw = 256 * acc
               }
             }
           }
