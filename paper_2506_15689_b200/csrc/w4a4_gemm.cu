@@ -5,22 +5,26 @@
 // The r1a kernel staged both operands packed -> smem -> unpack -> smem -> MMA and ran exactly at
 // the shared-memory bandwidth limit (144 KB of smem traffic per 128x256x128 k-block against a
 // 64 KB budget at the int8 MMA rate; profiles/r1a.md).  This version removes most of it:
-//   * the activation operand A never touches shared memory: four warps (thread = token row) load
-//     64 B of packed codes per k-block straight from global/L2 into registers, expand them and
-//     write int8 to TENSOR MEMORY with tcgen05.st; the MMA takes A from TMEM (.ts form);
+//   * the expanded activation operand A never touches shared memory: the packed codes arrive by
+//     TMA (SWIZZLE_64B), A warps (thread = token row) read them with conflict-free 16-byte LDS,
+//     expand them and write int8 to TENSOR MEMORY with tcgen05.st; the MMA takes A from TMEM
+//     (.ts form);
 //   * a CTA PAIR (cta_group::2, M = 256) shares the weight operand: each CTA stages and
 //     expands only half of the tile's N rows.
 // Per CTA and k-block the shared-memory traffic is  BN/2 x (64 B TMA write + 64 B unpack read +
-// 128 B unpack write + 128 B MMA read) = 36 KB at BN = 192  against 48 KB of budget.
+// 128 B unpack write + 128 B MMA read) = 36 KB at BN = 192, plus 16 KB for A's packed codes,
+// against 48 KB of budget.
 //
-// Persistent, warp-specialised, one CTA per SM, 512 threads:
-//   warp 0      B producer: one bulk-TMA copy per k-block of this CTA's weight box (packed ring)
-//   warp 1      MMA issuer (leader CTA of the pair only): 4 x tcgen05.mma.kind::i8 (K = 32) per
-//               k-block into one of two BN-column TMEM accumulators; commits multicast to both CTAs
-//   warps 4-7   epilogue: tcgen05.ld -> dequant (+ fused bias) -> bf16 -> global; overlaps the
-//               next tile's main loop through the second accumulator
-//   warps 8-11  A loaders (or, in the fused variant, the quantise-in-producer warps)
-//   warps 12-15 B unpackers: packed int4 -> int8 into SWIZZLE_128B K-major stages
+// Persistent, warp-specialised, one CTA per SM, 896 threads:
+//   warps 0, 2    TMA producers: A codes (2-D tensor map) / this CTA's weight box (bulk copy),
+//                 8-deep packed ring
+//   warp 1        MMA issuer (leader CTA of the pair only): 4 x tcgen05.mma.kind::i8 (K = 32) per
+//                 k-block into one of two BN-column TMEM accumulators; commits multicast to both CTAs
+//   warps 4-11    epilogue: tcgen05.ld -> dequant (+ fused bias) -> bf16 -> global; overlaps the
+//                 next tile's main loop through the second accumulator
+//   warps 12-19   A: LDS -> x16 expand -> tcgen05.st (two sets alternate k-blocks); in the fused
+//                 variant these eight warps quantise bf16 X instead (quant_math.cuh)
+//   warps 20-27   B: packed int4 -> int8 into SWIZZLE_128B K-major stages (two sets)
 //
 // x16 unpack: for a 32-bit word w holding 8 two's-complement nibbles,
 //   lo = (w << 4) & 0xF0F0F0F0   -> 4 signed bytes = 16 * (even-k codes)
