@@ -67,7 +67,7 @@ BASEQ_API int baseq_version(void);
  *   q_k = clamp(rne(u_k * (1 / s_t)), -8, 7)                                          (C-5, C-6)
  * every line one correctly rounded fp32 operation. */
 typedef struct {
-  float alpha;      /* clip ratio, 0 < alpha <= 1, else BASEQ_ERR_PARAM          */
+  float alpha;      /* clip ratio, 2^-16 <= alpha <= 1, else BASEQ_ERR_PARAM     */
   float gamma;      /* scalar s^a, used iff sa == NULL; must be finite and > 0                      */
   const float* sa;  /* [K] per-channel s^a, already divided by the paired scale s; or NULL          */
   const float* b;   /* [K] correction bias b^c in the scaled (and rotated) domain; NULL = 0         */

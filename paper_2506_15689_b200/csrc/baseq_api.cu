@@ -49,7 +49,7 @@ baseq_status_t check_shape(int T, int N, int K) {
 
 baseq_status_t check_act_params(const baseq_act_params_t* p, int K) {
   if (p == nullptr) return BASEQ_ERR_NULL;
-  if (!(p->alpha > 0.0f) || !(p->alpha <= 1.0f)) return BASEQ_ERR_PARAM;
+  if (!(p->alpha >= 1.0f / 65536.0f) || !(p->alpha <= 1.0f)) return BASEQ_ERR_PARAM;
   if (p->sa == nullptr && (!(p->gamma > 0.0f) || !std::isfinite(p->gamma))) return BASEQ_ERR_PARAM;
   if (p->had_block != 0) {
     const int B = p->had_block;

@@ -80,6 +80,15 @@ __device__ __forceinline__ void load_gb(const float* __restrict__ sa, const floa
   }
 }
 
+// 8 consecutive floats, loaded ONCE: asm volatile keeps ptxas from re-issuing the loads inside a
+// loop instead of holding the values in registers.
+__device__ __forceinline__ void load8_pinned(const float* __restrict__ p, float (&v)[8]) {
+  asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "l"(p));
+  asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]) : "l"(p + 4));
+}
+
 // Q2: u = fma(g, h, -b)
 __device__ __forceinline__ float affine(float g, float h, float b) { return __fmaf_rn(g, h, -b); }
 
@@ -109,13 +118,12 @@ __device__ __forceinline__ uint32_t pack_nibbles(const uint32_t (&t)[8]) {
 }
 
 
-// Q6 + Q7 for 8 channels at once.  Only the lower clamp is done in floating point; the magic add
-// rounds (RNE), an integer subtract recovers the signed code and cvt.pack.sat.s4.s32 saturates to
+// Q6 + Q7 for 8 channels at once.  |u * inv| <= 7 / alpha (1 + 2^-22) <= 7 * 2^16 < 2^22 because
+// |u| <= the row's absmax and the API requires alpha >= 2^-16, so the magic add is exact (RNE), the
+// integer subtract recovers the signed integer rne(r), and cvt.pack.sat.s4.s32 clamps it to
 // [-8, 7] and packs two codes per instruction:  d = (c << 8) | (sat(a) << 4) | (sat(b) & 15).
-// For r >= 2^22 the magic add is no longer exact but stays a large positive integer, which
-// saturates to 7 as required.
 __device__ __forceinline__ int32_t code_int(float u, float inv) {
-  const float r = fmaxf(__fmul_rn(u, inv), -8.0f);
+  const float r = __fmul_rn(u, inv);
   return static_cast<int32_t>(__float_as_uint(__fadd_rn(r, 12582912.0f))) - 0x4B400000;
 }
 __device__ __forceinline__ uint32_t pack2_sat(int32_t hi, int32_t lo, uint32_t prev) {

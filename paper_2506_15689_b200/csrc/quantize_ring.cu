@@ -94,9 +94,12 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
 #pragma unroll
     for (int i = 0; i < V; ++i) {
       const int idx = r + i * kConsumers;
-      float g_unused[8];
-      qm::load_gb(nullptr, p.bvec, p.gamma, idx, !RAGGED || idx < p.nvec, g_unused,
-                  bb[kBiasInRegs ? i : 0]);
+      if (p.bvec != nullptr && (!RAGGED || idx < p.nvec)) {
+        qm::load8_pinned(p.bvec + 8 * idx, bb[kBiasInRegs ? i : 0]);
+      } else {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) bb[kBiasInRegs ? i : 0][e] = 0.0f;
+      }
     }
   }
 
