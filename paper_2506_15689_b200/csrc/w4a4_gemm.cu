@@ -160,23 +160,22 @@ __device__ __noinline__ uint32_t dequant_f64(int32_t acc, float st, float sw, fl
 // `raw` is the TMEM accumulator 256 * acc (|acc| < 2^22, so raw has at most 22 significant bits
 // and converts to fp32 exactly) and st256 = s_t * 2^-8 (exact): st256 * float(raw) is the same
 // real number as s_t * acc and rounds to the same t.
-__device__ __forceinline__ uint32_t dequant_bf16(int32_t raw, float st256, float st, float sw,
-                                                 float fb) {
+// Branch-free fast path: returns the packed pair (bf16(hi) << 16) | bf16(lo) of the bracket ends
+//   hi, lo = y +- 2^-23 (|p| + |y| + 2^-100)
+// (the 2^-100 keeps the bracket wider than the absolute rounding errors when y is denormal).
+// The element is settled iff both halves are equal; `unsettled` accumulates (pk ^ swapped halves).
+__device__ __forceinline__ uint32_t dequant_bracket(int32_t raw, float st256, float sw, float fb,
+                                                    uint32_t& unsettled) {
   const float t = __fmul_rn(st256, __int2float_rn(raw));
   const float p = __fmul_rn(t, sw);
   const float y = __fmaf_rn(t, sw, fb);
-  const float s = __fadd_rn(fabsf(p), fabsf(y));
-  const float hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);     // y + 2^-23 (|p| + |y|)
+  const float s = __fadd_rn(__fadd_rn(fabsf(p), 7.888609052210118e-31f), fabsf(y));
+  const float hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);
   const float lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
   uint32_t pk;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));   // hi -> upper half
-  const uint32_t a = pk & 0xFFFFu, b = pk >> 16;
-  if (a == b && fabsf(y) > 1e-30f) return a;
-  return dequant_f64(raw >> 8, st, sw, fb);
-}
-__device__ __forceinline__ uint32_t dequant_bf16x2(int32_t r0, int32_t r1, float st256, float st,
-                                                   float2 sw, float2 fb) {
-  return dequant_bf16(r0, st256, st, sw.x, fb.x) | (dequant_bf16(r1, st256, st, sw.y, fb.y) << 16);
+  unsettled |= pk ^ __byte_perm(pk, 0, 0x1032);                          // halves swapped
+  return pk;
 }
 
 // ------------------------------------------------------------------------------ the kernel
@@ -538,13 +537,32 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
         ptx::tmem_ld_32x32b_x16(taddr + c0, r);
         ptx::tmem_ld_wait();
         uint32_t out[8];
+        uint32_t unsettled = 0;
 #pragma unroll
         for (int j = 0; j < 16; j += 2) {
           const int n = n0 + c0 + j;
           const float2 sw = __ldg(reinterpret_cast<const float2*>(p.sw + n));
           const float2 fb = __ldg(reinterpret_cast<const float2*>(p.fb + n));
-          out[j >> 1] = dequant_bf16x2(static_cast<int32_t>(r[j]), static_cast<int32_t>(r[j + 1]),
-                                       st256, st, sw, fb);
+          const uint32_t k0 = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw.x, fb.x, unsettled);
+          const uint32_t k1 = dequant_bracket(static_cast<int32_t>(r[j + 1]), st256, sw.y, fb.y, unsettled);
+          out[j >> 1] = __byte_perm(k0, k1, 0x5410);                  // low halves: lo0 | lo1 << 16
+        }
+        if (unsettled != 0) {
+          // rare (about 2.4e-4 of the elements): redo the chunk's unsettled elements with the fp64
+          // expression itself
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const int n = n0 + c0 + j;
+            const float sw = __ldg(p.sw + n), fb = __ldg(p.fb + n);
+            uint32_t dummy = 0;
+            const uint32_t k = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw, fb, dummy);
+            if (dummy != 0) {
+              const uint32_t v = dequant_f64(static_cast<int32_t>(r[j]) >> 8, st, sw, fb);
+              out[j >> 1] = (j & 1) ? ((out[j >> 1] & 0x0000FFFFu) | (v << 16))
+                                    : ((out[j >> 1] & 0xFFFF0000u) | v);
+            }
+            (void)k;
+          }
         }
         if (row_ok) {
 #pragma unroll
