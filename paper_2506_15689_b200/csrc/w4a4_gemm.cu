@@ -539,13 +539,16 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
         uint32_t out[8];
         uint32_t unsettled = 0;
 #pragma unroll
-        for (int j = 0; j < 16; j += 2) {
+        for (int j = 0; j < 16; j += 4) {
           const int n = n0 + c0 + j;
-          const float2 sw = __ldg(reinterpret_cast<const float2*>(p.sw + n));
-          const float2 fb = __ldg(reinterpret_cast<const float2*>(p.fb + n));
+          const float4 sw = __ldg(reinterpret_cast<const float4*>(p.sw + n));
+          const float4 fb = __ldg(reinterpret_cast<const float4*>(p.fb + n));
           const uint32_t k0 = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw.x, fb.x, unsettled);
           const uint32_t k1 = dequant_bracket(static_cast<int32_t>(r[j + 1]), st256, sw.y, fb.y, unsettled);
+          const uint32_t k2 = dequant_bracket(static_cast<int32_t>(r[j + 2]), st256, sw.z, fb.z, unsettled);
+          const uint32_t k3 = dequant_bracket(static_cast<int32_t>(r[j + 3]), st256, sw.w, fb.w, unsettled);
           out[j >> 1] = __byte_perm(k0, k1, 0x5410);                  // low halves: lo0 | lo1 << 16
+          out[(j >> 1) + 1] = __byte_perm(k2, k3, 0x5410);
         }
         if (unsettled != 0) {
           // rare (about 2.4e-4 of the elements): redo the chunk's unsettled elements with the fp64
