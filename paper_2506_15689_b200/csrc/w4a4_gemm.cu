@@ -163,9 +163,8 @@ __device__ __noinline__ uint32_t dequant_f64(int32_t acc, float st, float sw, fl
 // Branch-free fast path: returns the packed pair (bf16(hi) << 16) | bf16(lo) of the bracket ends
 //   hi, lo = y +- 2^-23 (|p| + |y| + 2^-100)
 // (the 2^-100 keeps the bracket wider than the absolute rounding errors when y is denormal).
-// The element is settled iff both halves are equal; `unsettled` accumulates (pk ^ swapped halves).
-__device__ __forceinline__ uint32_t dequant_bracket(int32_t raw, float st256, float sw, float fb,
-                                                    uint32_t& unsettled) {
+// The element is settled iff both halves are equal.
+__device__ __forceinline__ uint32_t dequant_bracket(int32_t raw, float st256, float sw, float fb) {
   const float t = __fmul_rn(st256, __int2float_rn(raw));
   const float p = __fmul_rn(t, sw);
   const float y = __fmaf_rn(t, sw, fb);
@@ -174,8 +173,15 @@ __device__ __forceinline__ uint32_t dequant_bracket(int32_t raw, float st256, fl
   const float lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
   uint32_t pk;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));   // hi -> upper half
-  unsettled |= pk ^ __byte_perm(pk, 0, 0x1032);                          // halves swapped
   return pk;
+}
+// two bracket pairs -> the output word bf16(lo0) | bf16(lo1) << 16; `unsettled` collects the
+// difference between the word of the low ends and the word of the high ends
+__device__ __forceinline__ uint32_t settle2(uint32_t k0, uint32_t k1, uint32_t& unsettled) {
+  const uint32_t los = __byte_perm(k0, k1, 0x5410);
+  const uint32_t his = __byte_perm(k0, k1, 0x7632);
+  unsettled |= los ^ his;
+  return los;
 }
 
 // ------------------------------------------------------------------------------ the kernel
@@ -543,12 +549,12 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           const int n = n0 + c0 + j;
           const float4 sw = __ldg(reinterpret_cast<const float4*>(p.sw + n));
           const float4 fb = __ldg(reinterpret_cast<const float4*>(p.fb + n));
-          const uint32_t k0 = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw.x, fb.x, unsettled);
-          const uint32_t k1 = dequant_bracket(static_cast<int32_t>(r[j + 1]), st256, sw.y, fb.y, unsettled);
-          const uint32_t k2 = dequant_bracket(static_cast<int32_t>(r[j + 2]), st256, sw.z, fb.z, unsettled);
-          const uint32_t k3 = dequant_bracket(static_cast<int32_t>(r[j + 3]), st256, sw.w, fb.w, unsettled);
-          out[j >> 1] = __byte_perm(k0, k1, 0x5410);                  // low halves: lo0 | lo1 << 16
-          out[(j >> 1) + 1] = __byte_perm(k2, k3, 0x5410);
+          const uint32_t k0 = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw.x, fb.x);
+          const uint32_t k1 = dequant_bracket(static_cast<int32_t>(r[j + 1]), st256, sw.y, fb.y);
+          const uint32_t k2 = dequant_bracket(static_cast<int32_t>(r[j + 2]), st256, sw.z, fb.z);
+          const uint32_t k3 = dequant_bracket(static_cast<int32_t>(r[j + 3]), st256, sw.w, fb.w);
+          out[j >> 1] = settle2(k0, k1, unsettled);
+          out[(j >> 1) + 1] = settle2(k2, k3, unsettled);
         }
         if (unsettled != 0) {
           // rare (about 2.4e-4 of the elements): redo the chunk's unsettled elements with the fp64
@@ -557,14 +563,12 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           for (int j = 0; j < 16; ++j) {
             const int n = n0 + c0 + j;
             const float sw = __ldg(p.sw + n), fb = __ldg(p.fb + n);
-            uint32_t dummy = 0;
-            const uint32_t k = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw, fb, dummy);
-            if (dummy != 0) {
+            const uint32_t k = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw, fb);
+            if ((k >> 16) != (k & 0xFFFFu)) {
               const uint32_t v = dequant_f64(static_cast<int32_t>(r[j]) >> 8, st, sw, fb);
               out[j >> 1] = (j & 1) ? ((out[j >> 1] & 0x0000FFFFu) | (v << 16))
                                     : ((out[j >> 1] & 0xFFFF0000u) | v);
             }
-            (void)k;
           }
         }
         if (row_ok) {
