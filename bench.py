@@ -101,7 +101,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(k)
             except Exception:
                 pass
-            self._stop_evt.wait(0.005)
+            self._stop_evt.wait(0.001)
 
     def stop(self):
         self._stop_evt.set()
