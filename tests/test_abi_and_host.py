@@ -110,3 +110,47 @@ def test_product_never_imports_the_oracle():
                 src = open(os.path.join(dirpath, fn)).read()
                 assert "import oracle" not in src and "from oracle" not in src, fn
                 assert "_work/" not in src, fn
+
+
+# ------------------------------------------------------------------------------- input recipe
+def _kurtosis(a):
+    a = a - a.mean()
+    return float((a ** 4).mean() / (a ** 2).mean() ** 2)
+
+
+def test_input_recipe_statistics():
+    """The seeded generators have the value statistics DESIGN.md section 4 states."""
+    from baseq_inputs import CONFIGS, make_activations, make_weights
+    from baseq_inputs.synth import bf16_bits_to_f32, unpack_nibbles
+    # c3 down: SiLU-gated product, heavy-tailed (kurtosis about 10)
+    A = make_activations("c3", "x_down", T=64)
+    x = bf16_bits_to_f32(A["x"]).astype(np.float64)
+    assert 7.0 < _kurtosis(x - x.mean(axis=0, keepdims=True)) < 14.0
+    # c5: Laplace(0, 1) around per-channel means (kurtosis 6, variance 2)
+    A5 = make_activations("c5", "x_down", T=32)
+    x5 = bf16_bits_to_f32(A5["x"]).astype(np.float64)
+    c5 = x5 - bf16_bits_to_f32(A5["calib"]).astype(np.float64).mean(axis=0, keepdims=True)
+    assert 4.5 < _kurtosis(c5) < 7.5 and 1.7 < c5.var() < 2.4
+    assert A5["b"].shape == (28672,) and A5["b"].dtype == np.float32
+    # c1: four outlier channels x20 (Eq. 1), b = column mean of gamma * X
+    A1 = make_activations("c1", "x")
+    x1 = bf16_bits_to_f32(A1["x"]).astype(np.float64)
+    std = x1.std(axis=0)
+    assert set(np.argsort(std)[-4:]) == {17, 101, 170, 233}
+    assert np.allclose(A1["b"], (1.05 * x1).mean(axis=0), rtol=0, atol=1e-5)
+    # weights: per-output-channel symmetric RTN int4 of N(0, 0.02^2): codes in [-8, 7], max |q| = 7
+    W = make_weights("c1", "linear")
+    q = unpack_nibbles(W["w_nibbles"])
+    assert q.min() >= -8 and q.max() <= 7 and np.all(np.abs(q).max(axis=1) == 7)
+    assert 0.005 < float(W["w_scale"].mean()) < 0.012      # ~ 0.02 * E[max of 256 |N(0,1)|] / 7
+    # shapes follow BASELINE.json
+    assert [(s.T, s.K, s.N) for s in CONFIGS["c3"]] == [(4096, 4096, 11008)] * 2 + [(4096, 11008, 4096)]
+    assert (CONFIGS["c5"][0].T, CONFIGS["c5"][0].K, CONFIGS["c5"][0].N, CONFIGS["c5"][0].had_block) == \
+        (4096, 28672, 8192, 128)
+
+
+def test_generators_are_deterministic():
+    from baseq_inputs import make_activations
+    a = make_activations("c2", "x", T=8)
+    b = make_activations("c2", "x", T=8)
+    assert np.array_equal(a["x"], b["x"]) and np.array_equal(a["b"], b["b"])
