@@ -242,6 +242,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
   const int num_tiles = p.num_m * p.num_n;
   const int first_tile = static_cast<int>(blockIdx.x) / CG;
   const int tile_step = static_cast<int>(gridDim.x) / CG;
+  const int n_it = first_tile < num_tiles
+                       ? ((num_tiles - first_tile + tile_step - 1) / tile_step) * p.num_kb : 0;
 
   if ((warp == kProducerWarp && !FUSED) || warp == kProducerWarpB) {
     // ===================================================================== producers (TMA)
@@ -335,19 +337,15 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     // ===================================================================== B: int4 -> int8
     const int ut = (threadIdx.x - kUnpackWarp0 * 32) & 127;   // 0..127 inside the set
     const int set = (warp - kUnpackWarp0) >> 2;
-    int it = 0;
-    int ps = 0, us = 0;
-    uint32_t pphase = 0, uphase = 0;
     constexpr int kTasks = C::kBRows * 4 / (kNumUnpackWarps * 32);   // 16-byte chunks per thread
     static_assert(C::kBRows * 4 % (kNumUnpackWarps * 32) == 0, "unpack tasks");
     const uint32_t full_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->full[0]), 0);
-    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-      for (int kb = 0; kb < p.num_kb; ++kb, ++it) {
-        if ((it & (kSets - 1)) != set) {
-          advance(ps, pphase, C::kPStages);
-          advance(us, uphase, kStages);
-          continue;
-        }
+    // flat k-block index over all of this CTA's tiles; this set takes every kSets-th one (the
+    // operand warps never need the tile coordinates)
+    {
+      for (int it = set; it < n_it; it += kSets) {
+        const int ps = it % C::kPStages, us = it % kStages;
+        const uint32_t pphase = (it / C::kPStages) & 1u, uphase = (it / kStages) & 1u;
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
         const uint8_t* src = packed_ptr + ps * C::kPackedStage + C::kPackedAArea;
         uint4 v[kTasks];
@@ -375,8 +373,6 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           ptx::mbar_arrive(ptx::smem_u32(&bars->pempty[ps]));
           ptx::mbar_arrive_cluster(full_remote + us * 8);
         }
-        advance(ps, pphase, C::kPStages);
-        advance(us, uphase, kStages);
       }
     }
   } else if (FUSED && warp >= kAWarp0 && warp < kAWarp0 + 8) {
@@ -475,16 +471,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     const uint32_t a_taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + kACol0;
     const int sw = (arow >> 1) & 3;
     const int set = (warp - kAWarp0) >> 2;
-    int it = 0;
-    int ps = 0, us = 0;
-    uint32_t pphase = 0, uphase = 0;
-    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-      for (int kb = 0; kb < p.num_kb; ++kb, ++it) {
-        if ((it & (kSets - 1)) != set) {
-          advance(ps, pphase, C::kPStages);
-          advance(us, uphase, kStages);
-          continue;
-        }
+    {
+      for (int it = set; it < n_it; it += kSets) {
+        const int ps = it % C::kPStages, us = it % kStages;
+        const uint32_t pphase = (it / C::kPStages) & 1u, uphase = (it / kStages) & 1u;
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
         const uint8_t* src = packed_ptr + ps * C::kPackedStage + arow * 64;
         uint4 w4[4];
@@ -510,8 +500,6 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           // the store consumed every lane's smem reads: the packed stage may be refilled
           ptx::mbar_arrive(ptx::smem_u32(&bars->pempty[ps]));
         }
-        advance(ps, pphase, C::kPStages);
-        advance(us, uphase, kStages);
       }
     }
   } else if (warp >= kEpiWarp0 && warp < kEpiWarp0 + kEpiWarps) {
