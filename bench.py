@@ -277,10 +277,13 @@ def run_gpu(args):
     quant_bytes = sum(kd[2] for kd in kernels if kd[0] == "quant")
     tops = gemm_ops / (gemm_ms * 1e-3) / 1e12
     int8_peak = 2.0 * peaks["bf16_sustained"]
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic = None     # dram bytes per launch of the dominant kernel, from the ncu capture in profiles/
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("w4a4_gemm_kernel_bytes_per_launch")
+        for ln in open(tpath).read().splitlines()[1:]:
+            f = ln.split(",")
+            if f[0] == "w4a4_gemm_kernel" and f[1].startswith("average"):
+                traffic = int(f[2])
     roofline = {"bound": "tensor", "kernel": "w4a4_gemm_kernel", "achieved": tops, "peak": int8_peak,
                 "unit": "TFLOP/s", "frac": tops / int8_peak, "traffic": traffic,
                 "peak_source": "2 x %s bf16 sustained (%s MEASURED_PEAKS.json; int8:bf16 nominal ratio 2)"

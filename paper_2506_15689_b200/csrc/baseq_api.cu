@@ -1,7 +1,6 @@
 // extern "C" entry points of libbaseq (include/baseq.h): host-side validation + dispatch.
 // No compute happens here and nothing falls back to the CPU.
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 
 #include "../../include/baseq.h"
@@ -10,8 +9,6 @@
 namespace {
 
 using namespace baseq;
-
-int quant_blocks_per_sm();
 
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
@@ -81,28 +78,8 @@ QuantLaunch make_quant(const void* x, int64_t ldx, int T, int K, const baseq_act
   q.tpr_log2 = 0;
   q.tpr_log2_override = 0;
   q.num_sms = 148;          // overwritten by the callers from the device query
-  q.blocks_per_sm = quant_blocks_per_sm();
+  q.blocks_per_sm = 2;
   return q;
-}
-
-// Tuning hook for profiling runs only: resident quantiser blocks per SM (default 2).
-int quant_blocks_per_sm() {
-  static int v = 0;
-  if (v == 0) {
-    const char* e = std::getenv("BASEQ_QUANT_BLOCKS_PER_SM");
-    v = (e != nullptr && e[0] >= '1' && e[0] <= '8') ? e[0] - '0' : 2;
-  }
-  return v;
-}
-
-// Tuning hook for profiling runs only: BASEQ_GEMM_CTA_GROUP=1 selects the single-CTA tiles.
-int gemm_cta_group() {
-  static int v = 0;
-  if (v == 0) {
-    const char* e = std::getenv("BASEQ_GEMM_CTA_GROUP");
-    v = (e != nullptr && e[0] == '1') ? 1 : 2;
-  }
-  return v;
 }
 
 }  // namespace
@@ -202,7 +179,6 @@ baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const 
   g.acc_dump = acc_dump;
   g.stream = static_cast<cudaStream_t>(stream);
   g.num_sms = sms;
-  g.cta_group = gemm_cta_group();
   const cudaError_t e = launch_w4a4_gemm(g);
   if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
@@ -261,7 +237,6 @@ baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
   g.codes_dump = codes_dump;
   g.stream = static_cast<cudaStream_t>(stream);
   g.num_sms = sms;
-  g.cta_group = gemm_cta_group();
   e = launch_w4a4_gemm(g);
   if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;

@@ -94,7 +94,6 @@ struct GemmLaunch {
   uint8_t* codes_dump;     // optional [T, K/2]
   cudaStream_t stream;
   int num_sms;
-  int cta_group;           // 2 = CTA pairs (default), 1 = single CTA per tile (tuning hook)
 };
 // Returns cudaSuccess, or an error (cudaErrorNotSupported when the tensor map cannot be built).
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g);

@@ -343,8 +343,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     // flat k-block index over all of this CTA's tiles; this set takes every kSets-th one (the
     // operand warps never need the tile coordinates)
     {
-      for (int it = set; it < n_it; it += kSets) {
-        const int ps = it % C::kPStages, us = it % kStages;
+      for (uint32_t it = set; it < static_cast<uint32_t>(n_it); it += kSets) {
+        const uint32_t ps = it % C::kPStages, us = it % kStages;      // unsigned: plain masks
         const uint32_t pphase = (it / C::kPStages) & 1u, uphase = (it / kStages) & 1u;
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
         const uint8_t* src = packed_ptr + ps * C::kPackedStage + C::kPackedAArea;
@@ -472,8 +472,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     const int sw = (arow >> 1) & 3;
     const int set = (warp - kAWarp0) >> 2;
     {
-      for (int it = set; it < n_it; it += kSets) {
-        const int ps = it % C::kPStages, us = it % kStages;
+      for (uint32_t it = set; it < static_cast<uint32_t>(n_it); it += kSets) {
+        const uint32_t ps = it % C::kPStages, us = it % kStages;      // unsigned: plain masks
         const uint32_t pphase = (it / C::kPStages) & 1u, uphase = (it / kStages) & 1u;
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
         const uint8_t* src = packed_ptr + ps * C::kPackedStage + arow * 64;
@@ -655,7 +655,8 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   if (fused && g.had_block > 128) return cudaErrorNotSupported;   // 16 lanes hold 128 channels
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
-  const int cg = g.cta_group == 1 ? 1 : 2;
+  constexpr int cg = 2;   // CTA pairs; the kernel template keeps CG = 1 (one CTA per 128 x BN tile)
+                          // for reference, but it is not instantiated
 
   // A operand (unfused): codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows, SWIZZLE_64B;
   // rows beyond T are zero-filled by TMA, so a ragged last M tile needs no special case.
@@ -697,11 +698,9 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
     p.had_block = g.had_block;
     p.had_scale = g.had_scale;
     p.codes_dump = reinterpret_cast<uint32_t*>(g.codes_dump);
-    return cg == 2 ? launch_cg<2, true>(tmap_a, p, g.num_sms, g.stream)
-                   : launch_cg<1, true>(tmap_a, p, g.num_sms, g.stream);
+    return launch_cg<2, true>(tmap_a, p, g.num_sms, g.stream);
   }
-  return cg == 2 ? launch_cg<2, false>(tmap_a, p, g.num_sms, g.stream)
-                 : launch_cg<1, false>(tmap_a, p, g.num_sms, g.stream);
+  return launch_cg<2, false>(tmap_a, p, g.num_sms, g.stream);
 }
 
 }  // namespace baseq
