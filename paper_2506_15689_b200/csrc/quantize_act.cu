@@ -185,7 +185,10 @@ cudaError_t launch_hw(const QuantLaunch& q, int V) {
 int quant_max_k() { return 512 * kMaxV * 8; }
 
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes) {
-  if (quantize_ring_supported(q.K) && q.tpr_log2_override == 0) return launch_quantize_ring(q, write_codes);
+  // long rows with the scalar s^a (every benchmark shape): bulk-TMA ring kernel; a per-channel
+  // s^a vector takes the register-resident kernel below
+  if (quantize_ring_supported(q.K) && q.sa == nullptr && q.tpr_log2_override == 0)
+    return launch_quantize_ring(q, write_codes);
   const int nvec = q.K / 8;
   // smallest power-of-two threads-per-row (>= 32) with at most 4 vectors per thread (the fp32 row
   // segment plus the prefetched next segment must leave room for two 256-thread blocks per SM);

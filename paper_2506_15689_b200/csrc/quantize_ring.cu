@@ -29,7 +29,6 @@ struct RingParams {
   int64_t row_bytes_stride;
   int T, K, nvec;
   float alpha, gamma;
-  const float* sa;
   const float* bvec;
   int had_block;
   float had_scale;
@@ -125,15 +124,15 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
         float f[8];
         qm::unpack8(xv, f);
         if (HAD) qm::hadamard8(f, p.had_block, p.had_scale, lane);
-        float gl[8], bl[8];
-        if (p.sa != nullptr || !kBiasInRegs) {
-          qm::load_gb(p.sa, kBiasInRegs ? nullptr : p.bvec, p.gamma, idx, ok, gl, bl);
+        float bl[8];
+        if (!kBiasInRegs) {
+          float g_unused[8];
+          qm::load_gb(nullptr, p.bvec, p.gamma, idx, ok, g_unused, bl);
         }
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
-          const float gg = p.sa != nullptr ? gl[e] : p.gamma;
           const float bv = kBiasInRegs ? bb[kBiasInRegs ? i : 0][e] : bl[e];
-          u[j][i][e] = qm::affine(gg, f[e], bv);
+          u[j][i][e] = qm::affine(p.gamma, f[e], bv);          // scalar s^a only (see the launcher)
           m[j] = fmaxf(m[j], fabsf(u[j][i][e]));
         }
       }
@@ -217,7 +216,6 @@ cudaError_t launch_ring_r(const QuantLaunch& q) {
   p.nvec = q.K / 8;
   p.alpha = q.alpha;
   p.gamma = q.gamma;
-  p.sa = q.sa;
   p.bvec = q.b;
   p.had_block = q.had_block;
   p.had_scale = q.had_scale;
