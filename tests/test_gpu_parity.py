@@ -338,3 +338,22 @@ def test_config5_fused_hadamard_small_T():
     rng = np.random.default_rng(55)
     W = _rand_w(rng, 200, 28672, bias=False)
     run_fused(A["x"], W, 0.9, 1.0, A["b"], had_block=128)
+
+
+# ------------------------------------------------------------------------------- randomised sweep
+def test_random_shapes_and_parameters():
+    """Seeded random (T, K, N, alpha, gamma, Hadamard block, bias on/off) cases, both paths."""
+    rng = np.random.default_rng(20260604)
+    for case in range(14):
+        T = int(rng.integers(1, 400))
+        K = 128 * int(rng.integers(1, 24))
+        N = 8 * int(rng.integers(1, 80))
+        alpha = float(rng.choice([1.0, 0.9, 0.75, 0.5]))
+        gamma = float(rng.choice([1.0, 1.05, 1.2]))
+        pow2 = [b for b in (2, 8, 32, 128) if K % b == 0]
+        B = int(rng.choice([0, 0] + pow2))
+        x = rand_x(rng, T, K, spread=float(rng.choice([0.0, 0.5, 2.0])))
+        b = (0.5 * rng.standard_normal(K)).astype(np.float32) if rng.random() < 0.8 else None
+        W = _rand_w(rng, N, K, bias=bool(rng.random() < 0.5))
+        run_linear(x, W, alpha, gamma, b, had_block=B, with_bias=W["layer_bias"] is not None)
+        run_fused(x, W, alpha, gamma, b, had_block=B)
