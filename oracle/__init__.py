@@ -14,4 +14,8 @@ from .binding import (  # noqa: F401
     gemm_i32,
     epilogue,
     linear,
+    quantize_act_asym,
+    gemm_i32_asym,
+    epilogue_asym,
+    linear_asym,
 )

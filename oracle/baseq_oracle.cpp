@@ -253,6 +253,122 @@ int oracle_epilogue(const int32_t* acc, const float* scales, const float* w_scal
   return 0;
 }
 
-int oracle_version(void) { return 1; }
+
+// =======================================================================================
+// NEXT-1: per-token ASYMMETRIC dynamic int4 activations -- the setting the paper's
+// accuracy numbers use ("Activations are quantized with per-token asymmetric dynamic
+// quantization").  Eq. 4:  x_q = clip(round((x - z) / s), 0, 2^b - 1) * s + z  with
+// "z and s ... the quantization lower bound and step size"; z = alpha * min(group),
+// s = alpha * (max - min) / (2^b - 1), floor 1e-12.  Same scale-then-bias input u as the
+// symmetric quantizer (Q0-Q2), then, each line one correctly rounded fp32 operation:
+//   A1  mn = min_k u_k, mx = max_k u_k
+//   A2  s_t = fmaxf((alpha * (mx - mn)) / 15, 1e-12);  z_t = alpha * mn;  inv = 1 / s_t
+//   A3  q_k = clamp(rint((u_k - z_t) * inv), 0, 15)          (unsigned code)
+//   A4  byte j = q_2j | (q_2j+1 << 4)
+// Parity status: pinned (lattice row 0..15 -> z = 0, s = 1, codes = the integers;
+// constant row; reconstruction within s/2 for alpha = 1; reduces to an independent numpy
+// restatement) -- tests/test_oracle_pins.py.
+// =======================================================================================
+int oracle_quantize_act_asym(const uint16_t* x_bf16, int64_t ldx, int T, int K, float alpha,
+                             float gamma, const float* sa, const float* b, int had_block,
+                             uint8_t* codes, float* scales, float* zeros) {
+  if (T < 1 || K < 2 || (K & 1)) return 2;
+  if (!(alpha > 0.0f) || !(alpha <= 1.0f)) return 4;
+  if (had_block != 0) {
+    if (had_block < 2 || (had_block & (had_block - 1)) != 0 || K % had_block != 0) return 4;
+  }
+  std::vector<float> x(static_cast<size_t>(K));
+  std::vector<float> u(static_cast<size_t>(K));
+  for (int t = 0; t < T; ++t) {
+    for (int k = 0; k < K; ++k) x[k] = bf16_bits_to_float(x_bf16[static_cast<int64_t>(t) * ldx + k]);
+    if (had_block) oracle_hadamard_blocks(x.data(), K, had_block);
+    for (int k = 0; k < K; ++k) {
+      float g = sa ? sa[k] : gamma;
+      float bk = b ? b[k] : 0.0f;
+      u[k] = std::fmaf(g, x[k], -bk);
+    }
+    // A1
+    float mn = u[0], mx = u[0];
+    for (int k = 1; k < K; ++k) {
+      mn = std::fmin(mn, u[k]);
+      mx = std::fmax(mx, u[k]);
+    }
+    // A2
+    float d = mx - mn;
+    float ad = alpha * d;
+    float st = ad / 15.0f;
+    st = std::fmax(st, 1e-12f);
+    float z = alpha * mn;
+    float inv = 1.0f / st;
+    // A3, A4
+    for (int k = 0; k < K; k += 2) {
+      unsigned q2[2];
+      for (int j = 0; j < 2; ++j) {
+        float v = u[k + j] - z;
+        float r = v * inv;
+        float rr = std::nearbyintf(r);
+        if (rr < 0.0f) rr = 0.0f;
+        if (rr > 15.0f) rr = 15.0f;
+        q2[j] = static_cast<unsigned>(rr);
+      }
+      codes[static_cast<int64_t>(t) * (K / 2) + k / 2] = static_cast<uint8_t>(q2[0] | (q2[1] << 4));
+    }
+    scales[t] = st;
+    zeros[t] = z;
+  }
+  return 0;
+}
+
+// acc[t,n] = sum_k qa[t,k] * qw[n,k] with UNSIGNED activation codes 0..15 and signed weights;
+// wsum[n] = sum_k qw[n,k] (the term the lower bound z multiplies).  |acc| <= 120 K.
+int oracle_gemm_i32_asym(const uint8_t* codes, const uint8_t* w_nibbles, int T, int N, int K,
+                         int32_t* acc, int32_t* wsum) {
+  if (T < 1 || N < 1 || K < 2 || (K & 1)) return 2;
+  for (int n = 0; n < N; ++n) {
+    int32_t s = 0;
+    for (int k = 0; k < K; ++k) {
+      unsigned byte = w_nibbles[static_cast<int64_t>(n) * (K / 2) + k / 2];
+      s += nibble_to_int((k & 1) ? (byte >> 4) : byte);
+    }
+    wsum[n] = s;
+  }
+  for (int t = 0; t < T; ++t) {
+    for (int n = 0; n < N; ++n) {
+      int32_t s = 0;
+      for (int k = 0; k < K; ++k) {
+        unsigned ab = codes[static_cast<int64_t>(t) * (K / 2) + k / 2];
+        unsigned wb = w_nibbles[static_cast<int64_t>(n) * (K / 2) + k / 2];
+        int a = static_cast<int>((k & 1) ? (ab >> 4) : (ab & 0xFu));
+        int w = nibble_to_int((k & 1) ? (wb >> 4) : wb);
+        s += a * w;
+      }
+      acc[static_cast<int64_t>(t) * N + n] = s;
+    }
+  }
+  return 0;
+}
+
+// Dequantised activation a_k = s_t q_k + z_t, so  sum_k W_deq[n,k] a_k = s_t s_w acc + z_t s_w wsum:
+//   c   = fma((double)z_t * (double)s_w[n], (double)wsum[n], (double)fb[n])
+//   y64 = fma((double)s_t * (double)s_w[n], (double)acc, c);   Y = bf16_rne(y64)
+int oracle_epilogue_asym(const int32_t* acc, const int32_t* wsum, const float* scales,
+                         const float* zeros, const float* w_scale, const float* fb, int T, int N,
+                         uint16_t* y_bf16, double* y64_out) {
+  if (T < 1 || N < 1) return 2;
+  for (int t = 0; t < T; ++t) {
+    for (int n = 0; n < N; ++n) {
+      double sw = static_cast<double>(w_scale[n]);
+      double f = fb ? static_cast<double>(fb[n]) : 0.0;
+      double c = std::fma(static_cast<double>(zeros[t]) * sw, static_cast<double>(wsum[n]), f);
+      double y = std::fma(static_cast<double>(scales[t]) * sw,
+                          static_cast<double>(acc[static_cast<int64_t>(t) * N + n]), c);
+      if (y64_out) y64_out[static_cast<int64_t>(t) * N + n] = y;
+      y_bf16[static_cast<int64_t>(t) * N + n] = oracle_bf16_from_double(y);
+    }
+  }
+  return 0;
+}
+
+int oracle_version(void) { return 2; }
 
 }  // extern "C"

@@ -50,6 +50,17 @@ def _load():
         lib.oracle_epilogue.restype = c.c_int
         lib.oracle_epilogue.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
                                         c.c_int, c.c_int, c.c_void_p, c.c_void_p]
+        lib.oracle_quantize_act_asym.restype = c.c_int
+        lib.oracle_quantize_act_asym.argtypes = [c.c_void_p, c.c_int64, c.c_int, c.c_int, c.c_float,
+                                                 c.c_float, c.c_void_p, c.c_void_p, c.c_int,
+                                                 c.c_void_p, c.c_void_p, c.c_void_p]
+        lib.oracle_gemm_i32_asym.restype = c.c_int
+        lib.oracle_gemm_i32_asym.argtypes = [c.c_void_p, c.c_void_p, c.c_int, c.c_int, c.c_int,
+                                             c.c_void_p, c.c_void_p]
+        lib.oracle_epilogue_asym.restype = c.c_int
+        lib.oracle_epilogue_asym.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                                             c.c_void_p, c.c_void_p, c.c_int, c.c_int, c.c_void_p,
+                                             c.c_void_p]
         _lib = lib
     return _lib
 
@@ -153,3 +164,54 @@ def linear(x_bf16, w_nibbles, w_scale, fb, alpha, gamma=1.0, sa=None, b=None, ha
     acc = gemm_i32(codes, w_nibbles)
     y, y64 = epilogue(acc, scales, w_scale, fb, return_y64=True)
     return {"codes": codes, "scales": scales, "acc": acc, "y": y, "y64": y64}
+
+
+# ------------------------------------------------------------------ NEXT-1: asymmetric activations
+def quantize_act_asym(x_bf16, alpha, gamma=1.0, sa=None, b=None, had_block=0):
+    """Per-token asymmetric int4 (Eq. 4).  Returns (codes u8 [T,K/2] with UNSIGNED
+    nibbles, scales [T] f32, zeros [T] f32 = the lattice lower bounds z_t)."""
+    _chk(x_bf16, np.uint16, "x_bf16")
+    T, K = x_bf16.shape
+    _chk(sa, np.float32, "sa")
+    _chk(b, np.float32, "b")
+    codes = np.empty((T, K // 2), dtype=np.uint8)
+    scales = np.empty((T,), dtype=np.float32)
+    zeros = np.empty((T,), dtype=np.float32)
+    rc = _load().oracle_quantize_act_asym(_ptr(x_bf16), K, T, K, alpha, gamma, _ptr(sa), _ptr(b),
+                                          had_block, _ptr(codes), _ptr(scales), _ptr(zeros))
+    if rc:
+        raise ValueError("oracle_quantize_act_asym: invalid arguments (status %d)" % rc)
+    return codes, scales, zeros
+
+
+def gemm_i32_asym(codes, w_nibbles):
+    """Unsigned activation codes x signed weights.  Returns (acc [T,N] i32, wsum [N] i32)."""
+    _chk(codes, np.uint8, "codes")
+    _chk(w_nibbles, np.uint8, "w_nibbles")
+    T, Kh = codes.shape
+    N = w_nibbles.shape[0]
+    acc = np.empty((T, N), dtype=np.int32)
+    wsum = np.empty((N,), dtype=np.int32)
+    rc = _load().oracle_gemm_i32_asym(_ptr(codes), _ptr(w_nibbles), T, N, 2 * Kh, _ptr(acc), _ptr(wsum))
+    if rc:
+        raise ValueError("oracle_gemm_i32_asym: invalid arguments (status %d)" % rc)
+    return acc, wsum
+
+
+def epilogue_asym(acc, wsum, scales, zeros, w_scale, fb=None, return_y64=False):
+    T, N = acc.shape
+    y = np.empty((T, N), dtype=np.uint16)
+    y64 = np.empty((T, N), dtype=np.float64) if return_y64 else None
+    rc = _load().oracle_epilogue_asym(_ptr(acc), _ptr(wsum), _ptr(scales), _ptr(zeros), _ptr(w_scale),
+                                      _ptr(fb), T, N, _ptr(y), _ptr(y64))
+    if rc:
+        raise ValueError("oracle_epilogue_asym: invalid arguments (status %d)" % rc)
+    return (y, y64) if return_y64 else y
+
+
+def linear_asym(x_bf16, w_nibbles, w_scale, fb, alpha, gamma=1.0, sa=None, b=None, had_block=0):
+    codes, scales, zeros = quantize_act_asym(x_bf16, alpha, gamma, sa, b, had_block)
+    acc, wsum = gemm_i32_asym(codes, w_nibbles)
+    y, y64 = epilogue_asym(acc, wsum, scales, zeros, w_scale, fb, return_y64=True)
+    return {"codes": codes, "scales": scales, "zeros": zeros, "acc": acc, "wsum": wsum, "y": y,
+            "y64": y64}

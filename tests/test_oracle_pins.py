@@ -477,3 +477,79 @@ def test_golden_fixture_matches_oracle():
     out = oracle.linear(L["x"], L["w_nibbles"], L["w_scale"], fb, sp.alpha, sp.gamma, None, L["b"])
     for key in ("codes", "scales", "acc", "y"):
         assert hashlib.sha256(out[key].tobytes()).hexdigest() == g[key], key
+
+
+# =========================================================================== NEXT-1: asymmetric
+def ucodes(codes):
+    lo = (codes & 0xF).astype(np.int64)
+    hi = (codes >> 4).astype(np.int64)
+    out = np.empty((codes.shape[0], codes.shape[1] * 2), dtype=np.int64)
+    out[:, 0::2], out[:, 1::2] = lo, hi
+    return out
+
+
+def test_asym_lattice_rows_exact():
+    # group [0..15], b = 4, asymmetric, alpha = 1 -> z = 0, s = 1, codes = the integers
+    row = np.tile(np.arange(16, dtype=np.float32), (3, 8))
+    c, s, z = oracle.quantize_act_asym(bf16(row), 1.0)
+    assert np.all(s == 1.0) and np.all(z == 0.0)
+    assert np.array_equal(ucodes(c), row.astype(np.int64))
+    # shifted lattice: values -5 .. 10 -> z = -5, s = 1, codes = value + 5
+    c, s, z = oracle.quantize_act_asym(bf16(row - 5.0), 1.0)
+    assert np.all(s == 1.0) and np.all(z == -5.0)
+    assert np.array_equal(ucodes(c), row.astype(np.int64))
+
+
+def test_asym_constant_row_and_floor():
+    # degenerate all-equal group -> floor scale, value reproduced exactly by z
+    row = np.full((2, 128), 5.0, dtype=np.float32)
+    c, s, z = oracle.quantize_act_asym(bf16(row), 1.0)
+    assert np.all(s == np.float32(1e-12)) and np.all(z == 5.0) and np.all(ucodes(c) == 0)
+
+
+def test_asym_matches_independent_restatement_and_reconstructs():
+    rng = np.random.default_rng(5)
+    x = (rng.standard_normal((7, 256)) * 2.0 + 1.5).astype(np.float32)
+    xb = bf16(x)
+    xf = (xb.astype(np.uint32) << 16).view(np.float32)
+    b = (0.3 * rng.standard_normal(256)).astype(np.float32)
+    for alpha in (1.0, 0.9):
+        c, s, z = oracle.quantize_act_asym(xb, alpha, 1.05, None, b)
+        # independent numpy restatement, every op in float32 (Eq. 4)
+        u = (np.float64(np.float32(1.05)) * xf.astype(np.float64) - b.astype(np.float64)).astype(np.float32)
+        mn, mx = u.min(axis=1), u.max(axis=1)
+        st = np.maximum((np.float32(alpha) * (mx - mn)) / np.float32(15.0), np.float32(1e-12)).astype(np.float32)
+        zz = (np.float32(alpha) * mn).astype(np.float32)
+        inv = (np.float32(1.0) / st).astype(np.float32)
+        q = np.clip(np.rint(((u - zz[:, None]).astype(np.float32) * inv[:, None]).astype(np.float32)), 0, 15)
+        assert np.array_equal(s.view(np.uint32), st.view(np.uint32))
+        assert np.array_equal(z.view(np.uint32), zz.view(np.uint32))
+        assert np.array_equal(ucodes(c), q.astype(np.int64))
+        if alpha == 1.0:
+            # reconstruction: |s q + z - u| <= s / 2 for every element (nothing is clipped)
+            rec = s[:, None].astype(np.float64) * ucodes(c) + z[:, None].astype(np.float64)
+            assert np.all(np.abs(rec - u.astype(np.float64)) <= 0.5 * s[:, None] * (1 + 2.0 ** -18))
+
+
+def test_asym_gemm_and_epilogue_identity():
+    # sum_k Wdeq[n,k] (s q_k + z) == s s_w acc + z s_w wsum  (the algebra the epilogue relies on),
+    # brute force on a tiny shape with exact rational arithmetic
+    rng = np.random.default_rng(9)
+    T, K, N = 3, 64, 5
+    qa = rng.integers(0, 16, size=(T, K))
+    qw = rng.integers(-8, 8, size=(N, K))
+    codes = (qa[:, 0::2] | (qa[:, 1::2] << 4)).astype(np.uint8)
+    wn = ((qw[:, 0::2] & 0xF) | ((qw[:, 1::2] & 0xF) << 4)).astype(np.uint8)
+    acc, wsum = oracle.gemm_i32_asym(codes, wn)
+    assert np.array_equal(acc, qa @ qw.T) and np.array_equal(wsum, qw.sum(axis=1))
+    s = np.array([0.5, 0.25, 0.125], dtype=np.float32)
+    z = np.array([-1.0, 0.5, 2.0], dtype=np.float32)
+    sw = np.array([0.5, 1.0, 2.0, 0.25, 4.0], dtype=np.float32)
+    fb = np.array([1.0, -2.0, 0.0, 0.5, 3.0], dtype=np.float32)
+    y, y64 = oracle.epilogue_asym(acc, wsum, s, z, sw, fb, return_y64=True)
+    for t in range(T):
+        for n in range(N):
+            exact = sum(Fraction(float(sw[n])) * int(qw[n, k]) * (Fraction(float(s[t])) * int(qa[t, k])
+                        + Fraction(float(z[t]))) for k in range(K)) + Fraction(float(fb[n]))
+            assert Fraction(float(y64[t, n])) == exact          # powers of two: no rounding at all
+            assert y[t, n] == oracle.bf16_from_double(float(exact))
