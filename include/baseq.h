@@ -115,6 +115,24 @@ BASEQ_API baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scal
                                int T, int N, int K, void* y_bf16, int64_t ldy, int32_t* acc_dump,
                                void* stream);
 
+/* ---- NEXT-1: per-token ASYMMETRIC dynamic int4 activations (the paper's deployed setting,
+ * P:241 "per-token asymmetric dynamic quantization"; Eq. 4 P:74 with lower bound z and step s;
+ * z = alpha * min, s = alpha * (max - min) / 15, floor 1e-12) ----
+ *   u_k as above;  mn = min u, mx = max u
+ *   s_t = max((alpha * (mx - mn)) / 15, 1e-12);  z_t = alpha * mn
+ *   q_k = clamp(rne((u_k - z_t) * (1 / s_t)), 0, 15)            UNSIGNED codes, same nibble packing
+ *   zeros  [T] fp32 lattice lower bounds z_t
+ * The GEMM multiplies the unsigned codes by the signed weights (tcgen05 kind::i8, U8 x S8) and the
+ * epilogue adds the lower-bound term:  Y = bf16_rne( fma(s_t s_w, acc, fma(z_t s_w, wsum[n], fb[n])) )
+ * with wsum[n] = sum_k qw[n,k] from the packed blob (fp64 expression, one rounding to bf16).
+ * p->sa must be NULL (scalar gamma only), else BASEQ_ERR_UNSUPPORTED; there is no fused variant. */
+BASEQ_API baseq_status_t baseq_quantize_act_asym(const void* x_bf16, int64_t ldx, int T, int K,
+                                       const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                       float* zeros, void* stream);
+BASEQ_API baseq_status_t baseq_w4a4_gemm_asym(const uint8_t* codes, const float* scales,
+                                    const float* zeros, const void* packed_w, int T, int N, int K,
+                                    void* y_bf16, int64_t ldy, int32_t* acc_dump, void* stream);
+
 /* ---- fused variant: quantise inside the GEMM producer; int4 codes never reach HBM ----
  * A per-token absmax pre-pass writes scales_out, then one GEMM kernel whose producer warps read
  * bf16 X tiles, apply Hadamard / scale / bias / round with the known per-token scale and write

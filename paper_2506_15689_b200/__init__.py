@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     linear_host,
     pack_weights,
     quantize_act,
+    quantize_act_asym,
+    w4a4_gemm_asym,
     w4a4_gemm,
     EXPORTED_SYMBOLS,
 )

@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = [
     "baseq_status_string", "baseq_version", "baseq_packed_weight_bytes", "baseq_pack_weights",
     "baseq_set_fused_bias", "baseq_quantize_act", "baseq_w4a4_gemm",
     "baseq_fused_workspace_bytes", "baseq_linear_fused", "baseq_linear_host_scratch_bytes",
-    "baseq_linear_host",
+    "baseq_linear_host", "baseq_quantize_act_asym", "baseq_w4a4_gemm_asym",
 ]
 
 
@@ -68,6 +68,10 @@ def lib():
         L.baseq_linear_host_scratch_bytes.argtypes = [i32, i32, i32]
         L.baseq_linear_host.restype = i32
         L.baseq_linear_host.argtypes = [vp, i32, i32, c.POINTER(_ActParamsC), vp, i32, vp, vp, sz, vp]
+        L.baseq_quantize_act_asym.restype = i32
+        L.baseq_quantize_act_asym.argtypes = [vp, i64, i32, i32, c.POINTER(_ActParamsC), vp, vp, vp, vp]
+        L.baseq_w4a4_gemm_asym.restype = i32
+        L.baseq_w4a4_gemm_asym.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -149,6 +153,29 @@ def w4a4_gemm(codes, scales, pw, y=None, acc_dump=None):
         y = torch.empty((T, pw.N), dtype=torch.bfloat16, device=codes.device)
     _check(lib().baseq_w4a4_gemm(_p(codes), _p(scales), _p(pw.blob), T, pw.N, pw.K, _p(y),
                                  y.stride(0), _p(acc_dump), _stream()), "baseq_w4a4_gemm")
+    return y
+
+
+def quantize_act_asym(x, params):
+    """NEXT-1: per-token asymmetric int4.  Returns (codes [T,K/2] u8 unsigned nibbles, scales, zeros)."""
+    T, K = x.shape
+    assert x.dtype == torch.bfloat16 and x.stride(1) == 1
+    codes = torch.empty((T, K // 2), dtype=torch.uint8, device=x.device)
+    scales = torch.empty((T,), dtype=torch.float32, device=x.device)
+    zeros = torch.empty((T,), dtype=torch.float32, device=x.device)
+    cs = params.c_struct()
+    _check(lib().baseq_quantize_act_asym(_p(x), x.stride(0), T, K, ctypes.byref(cs), _p(codes),
+                                         _p(scales), _p(zeros), _stream()), "baseq_quantize_act_asym")
+    return codes, scales, zeros
+
+
+def w4a4_gemm_asym(codes, scales, zeros, pw, y=None, acc_dump=None):
+    T = codes.shape[0]
+    if y is None:
+        y = torch.empty((T, pw.N), dtype=torch.bfloat16, device=codes.device)
+    _check(lib().baseq_w4a4_gemm_asym(_p(codes), _p(scales), _p(zeros), _p(pw.blob), T, pw.N, pw.K,
+                                      _p(y), y.stride(0), _p(acc_dump), _stream()),
+           "baseq_w4a4_gemm_asym")
     return y
 
 

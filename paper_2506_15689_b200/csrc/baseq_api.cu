@@ -77,6 +77,8 @@ QuantLaunch make_quant(const void* x, int64_t ldx, int T, int K, const baseq_act
   q.stream = static_cast<cudaStream_t>(stream);
   q.tpr_log2 = 0;
   q.tpr_log2_override = 0;
+  q.zeros = nullptr;
+  q.asym = false;
   q.num_sms = 148;          // overwritten by the callers from the device query
   q.blocks_per_sm = 2;
   return q;
@@ -170,6 +172,64 @@ baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const 
   GemmLaunch g{};
   g.codes = codes;
   g.scales = scales;
+  g.blob = packed_w;
+  g.T = T;
+  g.N = N;
+  g.K = K;
+  g.y = y_bf16;
+  g.ldy = ldy;
+  g.acc_dump = acc_dump;
+  g.stream = static_cast<cudaStream_t>(stream);
+  g.num_sms = sms;
+  const cudaError_t e = launch_w4a4_gemm(g);
+  if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
+baseq_status_t baseq_quantize_act_asym(const void* x_bf16, int64_t ldx, int T, int K,
+                                       const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                       float* zeros, void* stream) {
+  baseq_status_t st = check_shape(T, 8, K);
+  if (st != BASEQ_OK) return st;
+  if (x_bf16 == nullptr || codes == nullptr || scales == nullptr || zeros == nullptr || p == nullptr)
+    return BASEQ_ERR_NULL;
+  if (K > quant_max_k()) return BASEQ_ERR_SHAPE;
+  st = check_act_params(p, K);
+  if (st != BASEQ_OK) return st;
+  if (p->sa != nullptr) return BASEQ_ERR_UNSUPPORTED;
+  if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4) || !aligned(zeros, 4))
+    return BASEQ_ERR_ALIGN;
+  if (ldx < K || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;
+  int sms = 0;
+  st = device_check(&sms);
+  if (st != BASEQ_OK) return st;
+  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
+  q.num_sms = sms;
+  q.zeros = zeros;
+  q.asym = true;
+  const cudaError_t e = launch_quantize_ring(q, true);
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
+baseq_status_t baseq_w4a4_gemm_asym(const uint8_t* codes, const float* scales, const float* zeros,
+                                    const void* packed_w, int T, int N, int K, void* y_bf16,
+                                    int64_t ldy, int32_t* acc_dump, void* stream) {
+  if (codes == nullptr || scales == nullptr || zeros == nullptr || packed_w == nullptr ||
+      y_bf16 == nullptr)
+    return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(T, N, K);
+  if (st != BASEQ_OK) return st;
+  if (K > 65536) return BASEQ_ERR_SHAPE;             // raw accumulator 256 * 120 * K must fit int32
+  if (!aligned(codes, 16) || !aligned(y_bf16, 16) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
+  if (acc_dump != nullptr && !aligned(acc_dump, 16)) return BASEQ_ERR_ALIGN;
+  if (ldy < N || (ldy % 8) != 0) return BASEQ_ERR_ALIGN;
+  int sms = 0;
+  st = device_check(&sms);
+  if (st != BASEQ_OK) return st;
+  GemmLaunch g{};
+  g.codes = codes;
+  g.scales = scales;
+  g.zeros = zeros;
   g.blob = packed_w;
   g.T = T;
   g.N = N;

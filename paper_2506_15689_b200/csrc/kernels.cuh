@@ -7,7 +7,9 @@
 namespace baseq {
 
 // ------------------------------------------------------------------ packed weight blob
-// [ header 128 B | s_w[Npad] f32 | fb[Npad] f32 | boxes ]
+// [ header 128 B | s_w[Npad] f32 | fb[Npad] f32 | wsum[Npad] f32 | boxes ]
+// wsum[n] = sum_k qw[n,k] (an exact integer, |wsum| <= 8 K < 2^24, stored as fp32): the term the
+// lattice lower bound z_t of the asymmetric activation quantiser multiplies (NEXT-1).
 // boxes: [Npad/kTileRows][K/128] boxes of kTileRows rows x 64 bytes (= 128 int4 along K),
 // row-major inside the box, so one (row group, k-block) box is contiguous and consecutive
 // k-blocks of one row group are adjacent -- each is fetched with a single bulk-TMA copy.
@@ -23,13 +25,13 @@ constexpr int kTileBytes = kTileRows * kTileK / 2;
 struct BlobHeader {
   uint32_t magic;
   int32_t N, K, Npad;
-  uint64_t off_sw, off_fb, off_tiles, total_bytes;
+  uint64_t off_sw, off_fb, off_wsum, off_tiles, total_bytes;
 };
 
 inline int blob_npad(int N) { return (N + kGemmBN - 1) / kGemmBN * kGemmBN; }
 inline size_t blob_bytes(int N, int K) {
   const size_t npad = static_cast<size_t>(blob_npad(N));
-  return kBlobHeaderBytes + npad * 4 * 2 + npad * static_cast<size_t>(K) / 2;
+  return kBlobHeaderBytes + npad * 4 * 3 + npad * static_cast<size_t>(K) / 2;
 }
 inline BlobHeader blob_header(int N, int K) {
   BlobHeader h{};
@@ -39,7 +41,8 @@ inline BlobHeader blob_header(int N, int K) {
   h.Npad = blob_npad(N);
   h.off_sw = kBlobHeaderBytes;
   h.off_fb = h.off_sw + static_cast<uint64_t>(h.Npad) * 4;
-  h.off_tiles = h.off_fb + static_cast<uint64_t>(h.Npad) * 4;
+  h.off_wsum = h.off_fb + static_cast<uint64_t>(h.Npad) * 4;
+  h.off_tiles = h.off_wsum + static_cast<uint64_t>(h.Npad) * 4;
   h.total_bytes = blob_bytes(N, K);
   return h;
 }
@@ -56,6 +59,8 @@ struct QuantLaunch {
   float had_scale;     // (float)(1 / sqrt((double)had_block)), computed on the host
   uint8_t* codes;      // [T, K/2]
   float* scales;       // [T]
+  float* zeros;        // [T] lattice lower bounds z_t (asymmetric variant), else nullptr
+  bool asym;           // NEXT-1: per-token asymmetric int4 (unsigned codes)
   cudaStream_t stream;
   int tpr_log2;            // filled by the launcher
   int tpr_log2_override;   // 0 = heuristic (tuning hook for profiling runs)
@@ -78,6 +83,7 @@ cudaError_t launch_set_fused_bias(void* blob, int N, int K, const float* fb, cud
 struct GemmLaunch {
   const uint8_t* codes;    // [T, K/2]   (unfused) or nullptr (fused)
   const float* scales;     // [T]
+  const float* zeros;      // [T] asymmetric variant (unsigned codes), else nullptr
   const void* blob;
   int T, N, K;
   void* y;                 // bf16 [T, ldy]

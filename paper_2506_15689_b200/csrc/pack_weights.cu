@@ -35,26 +35,31 @@ __global__ void retile_kernel(const uint8_t* __restrict__ w, int N, int K, int N
 __global__ void scales_bias_kernel(const uint8_t* __restrict__ w, const float* __restrict__ w_scale,
                                    const float* __restrict__ b, const float* __restrict__ bias,
                                    int N, int K, int Npad, float* __restrict__ sw_out,
-                                   float* __restrict__ fb_out, float* __restrict__ fb_copy) {
+                                   float* __restrict__ fb_out, float* __restrict__ wsum_out,
+                                   float* __restrict__ fb_copy) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n >= Npad) return;
   if (n >= N) {
     sw_out[n] = 0.0f;
     fb_out[n] = 0.0f;
+    wsum_out[n] = 0.0f;
     return;
   }
   double s = 0.0;
-  if (b != nullptr) {
-    const uint8_t* row = w + static_cast<int64_t>(n) * (K / 2);
-    for (int j = 0; j < K / 2; ++j) {
-      const uint32_t byte = row[j];
-      const int q0 = static_cast<int>(byte << 28) >> 28;        // sign-extend low nibble
-      const int q1 = static_cast<int>(byte << 24) >> 28;        // sign-extend high nibble
+  int wsum = 0;
+  const uint8_t* row = w + static_cast<int64_t>(n) * (K / 2);
+  for (int j = 0; j < K / 2; ++j) {
+    const uint32_t byte = row[j];
+    const int q0 = static_cast<int>(byte << 28) >> 28;        // sign-extend low nibble
+    const int q1 = static_cast<int>(byte << 24) >> 28;        // sign-extend high nibble
+    wsum += q0 + q1;
+    if (b != nullptr) {
       // q * b is exact in fp64, so fma(q, b, s) == s + q*b rounded once (same as the oracle)
       s = __fma_rn(static_cast<double>(q0), static_cast<double>(b[2 * j]), s);
       s = __fma_rn(static_cast<double>(q1), static_cast<double>(b[2 * j + 1]), s);
     }
   }
+  wsum_out[n] = static_cast<float>(wsum);                      // exact: |wsum| <= 8 K < 2^24
   double v = __dmul_rn(static_cast<double>(w_scale[n]), s);
   if (bias != nullptr) v = __dadd_rn(v, static_cast<double>(bias[n]));
   const float f = __double2float_rn(v);
@@ -93,7 +98,8 @@ cudaError_t launch_pack_weights(const uint8_t* w_nibbles, const float* w_scale, 
   if (e != cudaSuccess) return e;
   scales_bias_kernel<<<(h.Npad + 63) / 64, 64, 0, stream>>>(
       w_nibbles, w_scale, b, layer_bias, N, K, h.Npad, reinterpret_cast<float*>(base + h.off_sw),
-      reinterpret_cast<float*>(base + h.off_fb), fused_bias_out);
+      reinterpret_cast<float*>(base + h.off_fb), reinterpret_cast<float*>(base + h.off_wsum),
+      fused_bias_out);
   return cudaGetLastError();
 }
 

@@ -189,8 +189,9 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t smem_addr) {
 // Instruction descriptor for kind::i8, S8 x S8 -> S32, both operands K-major.
 // [4,6) D format (2 = S32), [7,10) A format (1 = S8), [10,13) B format (1 = S8),
 // [15] A major (0 = K), [16] B major (0 = K), [17,23) N>>3, [24,29) M>>4.
-__host__ __device__ constexpr uint32_t make_idesc_i8(uint32_t M, uint32_t N) {
-  return (2u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+// a_unsigned: A format U8 (0) instead of S8 (1) -- unsigned activation codes x signed weights.
+__host__ __device__ constexpr uint32_t make_idesc_i8(uint32_t M, uint32_t N, bool a_unsigned = false) {
+  return (2u << 4) | ((a_unsigned ? 0u : 1u) << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
 }
 
 // ---------------------------------------------------------------- global memory

@@ -138,5 +138,32 @@ __device__ __forceinline__ uint32_t quantize_pack8(const float (&u)[8], float in
   return pack2_sat(code_int(u[1], inv), code_int(u[0], inv), w);
 }
 
+
+// ---------------------------------------------------------------- NEXT-1: asymmetric (Eq. 4)
+//   A2  s_t = max((alpha * (mx - mn)) / 15, 1e-12);  z_t = alpha * mn;  inv = 1 / s_t
+//   A3  q   = clamp(rne((u - z_t) * inv), 0, 15)
+__device__ __forceinline__ float step_size_asym(float alpha, float mn, float mx) {
+  return fmaxf(__fdiv_rn(__fmul_rn(alpha, __fsub_rn(mx, mn)), 15.0f), 1e-12f);
+}
+__device__ __forceinline__ float lower_bound_asym(float alpha, float mn) { return __fmul_rn(alpha, mn); }
+// The lower clamp is done in floating point (rne is monotone and rne(0) = 0, so clamping before
+// rounding is the same thing; it also keeps the magic add away from its wrap-around), the upper
+// one by the saturating pack:  d = (c << 8) | (sat_u4(a) << 4) | sat_u4(b).
+__device__ __forceinline__ int32_t code_int_asym(float u, float z, float inv) {
+  const float r = fmaxf(__fmul_rn(__fsub_rn(u, z), inv), 0.0f);
+  return static_cast<int32_t>(__float_as_uint(__fadd_rn(r, 12582912.0f))) - 0x4B400000;
+}
+__device__ __forceinline__ uint32_t pack2_sat_u(int32_t hi, int32_t lo, uint32_t prev) {
+  uint32_t d;
+  asm("cvt.pack.sat.u4.s32.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(hi), "r"(lo), "r"(prev));
+  return d;
+}
+__device__ __forceinline__ uint32_t quantize_pack8_asym(const float (&u)[8], float z, float inv) {
+  uint32_t w = pack2_sat_u(code_int_asym(u[7], z, inv), code_int_asym(u[6], z, inv), 0u);
+  w = pack2_sat_u(code_int_asym(u[5], z, inv), code_int_asym(u[4], z, inv), w);
+  w = pack2_sat_u(code_int_asym(u[3], z, inv), code_int_asym(u[2], z, inv), w);
+  return pack2_sat_u(code_int_asym(u[1], z, inv), code_int_asym(u[0], z, inv), w);
+}
+
 }  // namespace qm
 }  // namespace baseq

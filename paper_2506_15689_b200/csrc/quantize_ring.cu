@@ -34,6 +34,7 @@ struct RingParams {
   float had_scale;
   uint32_t* codes;
   float* scales;
+  float* zeros;            // asymmetric variant only
   int stages;
   int stage_bytes;
 };
@@ -42,12 +43,14 @@ __device__ __forceinline__ void named_barrier_sync(int id, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
-template <int V, int RL, bool HAD, bool WRITE_CODES, bool RAGGED>
+template <int V, int RL, bool HAD, bool WRITE_CODES, bool RAGGED, bool ASYM>
 __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const RingParams p) {
   extern __shared__ __align__(128) uint8_t ring[];
   __shared__ uint64_t full[kMaxStages], empty[kMaxStages];
   __shared__ float s_part[2][RL][kConsumerWarps];
+  __shared__ float s_part2[ASYM ? 2 : 1][RL][kConsumerWarps];   // asymmetric: max(-u) = -min(u)
   __shared__ float2 s_scale[2][RL];
+  __shared__ float s_zero[2][RL];
 
   const int tid = threadIdx.x;
   const int warp = tid >> 5, lane = tid & 31;
@@ -112,9 +115,11 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
     // ---- pass 1: smem -> registers, Hadamard, u = g*h - b, absmax
     float u[RL][V][8];
     float m[RL];
+    float m2[RL];                                      // asymmetric only: running max of -u
 #pragma unroll
     for (int j = 0; j < RL; ++j) {
-      m[j] = 0.0f;
+      m[j] = ASYM ? -3.402823466e38f : 0.0f;
+      m2[j] = -3.402823466e38f;
 #pragma unroll
       for (int i = 0; i < V; ++i) {
         const int idx = r + i * kConsumers;
@@ -133,7 +138,14 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
         for (int e = 0; e < 8; ++e) {
           const float bv = kBiasInRegs ? bb[kBiasInRegs ? i : 0][e] : bl[e];
           u[j][i][e] = qm::affine(p.gamma, f[e], bv);          // scalar s^a only (see the launcher)
-          m[j] = fmaxf(m[j], fabsf(u[j][i][e]));
+          if (ASYM) {
+            if (ok) {
+              m[j] = fmaxf(m[j], u[j][i][e]);
+              m2[j] = fmaxf(m2[j], -u[j][i][e]);
+            }
+          } else {
+            m[j] = fmaxf(m[j], fabsf(u[j][i][e]));
+          }
         }
       }
     }
@@ -145,7 +157,20 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
     // ---- block reduction: warp shuffle -> partials -> one warp per row finishes.
     // RL row maxima are reduced together: each xor step that halves the live values costs one
     // shuffle per surviving value (6 shuffles for 4 rows instead of 20).
-    if (RL == 4) {
+    if (ASYM) {
+#pragma unroll
+      for (int j = 0; j < RL; ++j) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          m[j] = fmaxf(m[j], __shfl_xor_sync(0xffffffffu, m[j], o));
+          m2[j] = fmaxf(m2[j], __shfl_xor_sync(0xffffffffu, m2[j], o));
+        }
+        if (lane == 0) {
+          s_part[parity][j][warp] = m[j];
+          s_part2[ASYM ? parity : 0][j][warp] = m2[j];
+        }
+      }
+    } else if (RL == 4) {
       const bool up16 = (lane & 16) != 0, up8 = (lane & 8) != 0;
       float s0 = up16 ? m[0] : m[2], s1 = up16 ? m[1] : m[3];      // what the partner keeps
       float k0 = up16 ? m[2] : m[0], k1 = up16 ? m[3] : m[1];
@@ -176,13 +201,22 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
     }
     named_barrier_sync(1, kConsumers);
     if (warp < RL) {
-      float mm = lane < kConsumerWarps ? s_part[parity][warp][lane] : 0.0f;
+      float mm = lane < kConsumerWarps ? s_part[parity][warp][lane] : (ASYM ? -3.402823466e38f : 0.0f);
+      float mm2 = (ASYM && lane < kConsumerWarps) ? s_part2[ASYM ? parity : 0][warp][lane]
+                                                  : -3.402823466e38f;
 #pragma unroll
-      for (int o = 8; o > 0; o >>= 1) mm = fmaxf(mm, __shfl_xor_sync(0xffffffffu, mm, o));
+      for (int o = 8; o > 0; o >>= 1) {
+        mm = fmaxf(mm, __shfl_xor_sync(0xffffffffu, mm, o));
+        if (ASYM) mm2 = fmaxf(mm2, __shfl_xor_sync(0xffffffffu, mm2, o));
+      }
       if (lane == 0) {
-        const float st = qm::step_size(p.alpha, mm);
+        const float st = ASYM ? qm::step_size_asym(p.alpha, -mm2, mm) : qm::step_size(p.alpha, mm);
         s_scale[parity][warp] = make_float2(st, qm::reciprocal(st));
-        if (row0 + warp < p.T) p.scales[row0 + warp] = st;
+        if (ASYM) s_zero[parity][warp] = qm::lower_bound_asym(p.alpha, -mm2);
+        if (row0 + warp < p.T) {
+          p.scales[row0 + warp] = st;
+          if (ASYM) p.zeros[row0 + warp] = qm::lower_bound_asym(p.alpha, -mm2);
+        }
       }
     }
     named_barrier_sync(2, kConsumers);
@@ -197,7 +231,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
 #pragma unroll
           for (int i = 0; i < V; ++i) {
             const int idx = r + i * kConsumers;
-            const uint32_t w = qm::quantize_pack8(u[j][i], inv);
+            const uint32_t w = ASYM ? qm::quantize_pack8_asym(u[j][i], s_zero[parity][j], inv)
+                                    : qm::quantize_pack8(u[j][i], inv);
             if (!RAGGED || idx < p.nvec) crow[idx] = w;
           }
         }
@@ -206,8 +241,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
   }
 }
 
-template <int V, int RL, bool HAD, bool WC, bool RAGGED>
-cudaError_t launch_ring_r(const QuantLaunch& q) {
+template <int V, int RL, bool HAD, bool WC, bool RAGGED, bool ASYM>
+cudaError_t launch_ring_a(const QuantLaunch& q) {
   RingParams p{};
   p.x = static_cast<const uint8_t*>(q.x);
   p.row_bytes_stride = q.ldx * 2;
@@ -221,6 +256,7 @@ cudaError_t launch_ring_r(const QuantLaunch& q) {
   p.had_scale = q.had_scale;
   p.codes = reinterpret_cast<uint32_t*>(q.codes);
   p.scales = q.scales;
+  p.zeros = q.zeros;
   p.stage_bytes = RL * q.K * 2;
   int stages = kRingSmemBudget / p.stage_bytes;
   p.stages = stages > kMaxStages ? kMaxStages : stages;
@@ -228,15 +264,22 @@ cudaError_t launch_ring_r(const QuantLaunch& q) {
   const int smem = p.stages * p.stage_bytes;
   static int attr_smem = 0;
   if (smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(quantize_ring_kernel<V, RL, HAD, WC, RAGGED>,
+    cudaError_t e = cudaFuncSetAttribute(quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     attr_smem = smem;
   }
   const int groups = (q.T + RL - 1) / RL;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
-  quantize_ring_kernel<V, RL, HAD, WC, RAGGED><<<blocks, kRingThreads, smem, q.stream>>>(p);
+  quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM><<<blocks, kRingThreads, smem, q.stream>>>(p);
   return cudaGetLastError();
+}
+
+template <int V, int RL, bool HAD, bool WC, bool RAGGED>
+cudaError_t launch_ring_r(const QuantLaunch& q) {
+  // the asymmetric variant (NEXT-1) always writes codes
+  if (q.asym) return WC ? launch_ring_a<V, RL, HAD, true, RAGGED, true>(q) : cudaErrorInvalidValue;
+  return launch_ring_a<V, RL, HAD, WC, RAGGED, false>(q);
 }
 
 template <int V, int RL, bool HAD, bool WC>

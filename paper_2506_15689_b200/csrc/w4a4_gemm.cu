@@ -105,6 +105,8 @@ struct GemmParams {
   const float* sw;          // [Npad]
   const float* fb;          // [Npad]
   const float* scales;      // [T]
+  const float* zeros;       // [T] lattice lower bounds z_t (asymmetric variant)
+  const float* wsum;        // [Npad] sum_k qw[n,k] as fp32 (asymmetric variant)
   uint16_t* y;              // bf16 [T, ldy]
   int64_t ldy;
   int32_t* acc_dump;        // optional [T, N]
@@ -175,6 +177,18 @@ __device__ __forceinline__ uint32_t dequant_bracket(int32_t raw, float st256, fl
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));   // hi -> upper half
   return pk;
 }
+// Asymmetric variant: y* = (s_t s_w) acc + (z_t s_w) wsum + fb.  The two products are large and
+// nearly cancel (that is what a lower bound z_t far from zero means), so an fp32 evaluation's error
+// bracket is ~80x wider than |y| and almost never settles (measured: the bracketed version spent
+// most chunks in the fp64 fix-up).  The fp64 expression is therefore evaluated directly for every
+// element (5 DP operations + 2 conversions per output; B200's FP64 rate is half its FP32 rate).
+__device__ __forceinline__ uint32_t dequant_f64_asym(int32_t acc, double std_, double ztd, float sw,
+                                                     float fb, float ws) {
+  const double swd = static_cast<double>(sw);
+  const double c = __fma_rn(__dmul_rn(ztd, swd), static_cast<double>(ws), static_cast<double>(fb));
+  const double yd = __fma_rn(__dmul_rn(std_, swd), static_cast<double>(acc), c);
+  return bf16_from_double_rne(yd);
+}
 // two bracket pairs -> the output word bf16(lo0) | bf16(lo1) << 16; `unsettled` collects the
 // difference between the word of the low ends and the word of the high ends
 __device__ __forceinline__ uint32_t settle2(uint32_t k0, uint32_t k1, uint32_t& unsettled) {
@@ -186,7 +200,8 @@ __device__ __forceinline__ uint32_t settle2(uint32_t k0, uint32_t k1, uint32_t& 
 
 // ------------------------------------------------------------------------------ the kernel
 // CG = 1: one CTA per tile of 128 x BN;  CG = 2: a CTA pair per tile of 256 x BN.
-template <int CG, bool FUSED>
+// ASYM (NEXT-1): unsigned activation codes (A format U8) and the epilogue term z_t s_w wsum[n].
+template <int CG, bool FUSED, bool ASYM>
 __global__ void __launch_bounds__((Cfg<CG, FUSED>::kThreads), 1)
 w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   using C = Cfg<CG, FUSED>;
@@ -289,7 +304,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     // waterfall (~95 SASS instructions and ~670 clk per k-block, measured -- slower than the
     // 384 clk the four MMAs take).
     if (leader) {
-      constexpr uint32_t idesc = ptx::make_idesc_i8(BM * CG, BN);
+      constexpr uint32_t idesc = ptx::make_idesc_i8(BM * CG, BN, ASYM);
       int stage = 0, as = 0;
       uint32_t phase = 0, aphase = 0;
       const uint64_t desc0 = ptx::make_smem_desc_sw128(unpacked0);
@@ -518,6 +533,9 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       const bool row_ok = row < p.T;
       const float st = row_ok ? p.scales[row] : 0.0f;
       const float st256 = __fmul_rn(st, 0.00390625f);
+      const double std_ = static_cast<double>(st);
+      const double ztd = (ASYM && row_ok) ? static_cast<double>(p.zeros[row]) : 0.0;
+      (void)std_; (void)ztd;
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
       ptx::tcgen05_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN +
@@ -537,6 +555,16 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           const int n = n0 + c0 + j;
           const float4 sw = __ldg(reinterpret_cast<const float4*>(p.sw + n));
           const float4 fb = __ldg(reinterpret_cast<const float4*>(p.fb + n));
+          if (ASYM) {
+            const float4 ws = __ldg(reinterpret_cast<const float4*>(p.wsum + n));
+            const uint32_t v0 = dequant_f64_asym(static_cast<int32_t>(r[j]) >> 8, std_, ztd, sw.x, fb.x, ws.x);
+            const uint32_t v1 = dequant_f64_asym(static_cast<int32_t>(r[j + 1]) >> 8, std_, ztd, sw.y, fb.y, ws.y);
+            const uint32_t v2 = dequant_f64_asym(static_cast<int32_t>(r[j + 2]) >> 8, std_, ztd, sw.z, fb.z, ws.z);
+            const uint32_t v3 = dequant_f64_asym(static_cast<int32_t>(r[j + 3]) >> 8, std_, ztd, sw.w, fb.w, ws.w);
+            out[j >> 1] = v0 | (v1 << 16);
+            out[(j >> 1) + 1] = v2 | (v3 << 16);
+            continue;
+          }
           const uint32_t k0 = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw.x, fb.x);
           const uint32_t k1 = dequant_bracket(static_cast<int32_t>(r[j + 1]), st256, sw.y, fb.y);
           const uint32_t k2 = dequant_bracket(static_cast<int32_t>(r[j + 2]), st256, sw.z, fb.z);
@@ -619,13 +647,13 @@ EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-template <int CG, bool FUSED>
+template <int CG, bool FUSED, bool ASYM>
 cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sms,
                       cudaStream_t stream) {
   using C = Cfg<CG, FUSED>;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(w4a4_gemm_kernel<CG, FUSED>,
+    cudaError_t e = cudaFuncSetAttribute(w4a4_gemm_kernel<CG, FUSED, ASYM>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
     if (e != cudaSuccess) return e;
     attr_set = true;
@@ -645,7 +673,7 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sm
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG, FUSED>, tmap_a, p);
+  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG, FUSED, ASYM>, tmap_a, p);
 }
 
 }  // namespace
@@ -680,6 +708,8 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   p.sw = reinterpret_cast<const float*>(base + h.off_sw);
   p.fb = reinterpret_cast<const float*>(base + h.off_fb);
   p.scales = g.scales;
+  p.zeros = g.zeros;
+  p.wsum = reinterpret_cast<const float*>(base + h.off_wsum);
   p.y = static_cast<uint16_t*>(g.y);
   p.ldy = g.ldy;
   p.acc_dump = g.acc_dump;
@@ -698,9 +728,11 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
     p.had_block = g.had_block;
     p.had_scale = g.had_scale;
     p.codes_dump = reinterpret_cast<uint32_t*>(g.codes_dump);
-    return launch_cg<2, true>(tmap_a, p, g.num_sms, g.stream);
+    if (g.zeros != nullptr) return cudaErrorNotSupported;   // fused + asymmetric: not built
+    return launch_cg<2, true, false>(tmap_a, p, g.num_sms, g.stream);
   }
-  return launch_cg<2, false>(tmap_a, p, g.num_sms, g.stream);
+  if (g.zeros != nullptr) return launch_cg<2, false, true>(tmap_a, p, g.num_sms, g.stream);
+  return launch_cg<2, false, false>(tmap_a, p, g.num_sms, g.stream);
 }
 
 }  // namespace baseq

@@ -53,7 +53,7 @@ def test_size_queries_and_blob_layout():
     for N, K in [(8, 128), (256, 256), (4096, 4096), (11008, 4096), (8192, 28672)]:
         nb = L.baseq_packed_weight_bytes(N, K)
         npad = -(-N // 192) * 192                               # tile N extent
-        assert nb == 128 + 8 * npad + npad * K // 2
+        assert nb == 128 + 12 * npad + npad * K // 2
     assert L.baseq_fused_workspace_bytes(0, 8, 128) == 0
     assert L.baseq_fused_workspace_bytes(16, 256, 256) >= 1
     assert L.baseq_linear_host_scratch_bytes(16, 256, 256) >= 16 * 256 * 2 + 16 * 128 + 64 + 16 * 256 * 2

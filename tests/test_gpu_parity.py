@@ -357,3 +357,76 @@ def test_random_shapes_and_parameters():
         W = _rand_w(rng, N, K, bias=bool(rng.random() < 0.5))
         run_linear(x, W, alpha, gamma, b, had_block=B, with_bias=W["layer_bias"] is not None)
         run_fused(x, W, alpha, gamma, b, had_block=B)
+
+
+# ------------------------------------------------------------------------------- NEXT-1: asymmetric
+def run_asym(x_bits, W, alpha, gamma, b, had_block=0, rows=None):
+    """baseq_quantize_act_asym + baseq_w4a4_gemm_asym vs the oracle, everything bit for bit."""
+    N, K = W["N"], W["K"]
+    T = x_bits.shape[0]
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None if b is None else dev(b),
+                         None if W["layer_bias"] is None else dev(W["layer_bias"]))
+    params = bq.ActParams(alpha, gamma, None, None if b is None else dev(b), had_block)
+    codes, scales, zeros = bq.quantize_act_asym(bf16_dev(x_bits), params)
+    acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
+    y = bq.w4a4_gemm_asym(codes, scales, zeros, pw, acc_dump=acc)
+    y2 = bq.w4a4_gemm_asym(codes, scales, zeros, pw)
+    torch.cuda.synchronize()
+    assert torch.equal(y.view(torch.int16), y2.view(torch.int16))
+    sel = np.arange(T) if rows is None else rows
+    ref = oracle.linear_asym(np.ascontiguousarray(x_bits[sel]), W["w_nibbles"], W["w_scale"], fb,
+                             alpha, gamma, None, b, had_block)
+    assert np.array_equal(scales.cpu().numpy()[sel].view(np.uint32), ref["scales"].view(np.uint32))
+    assert np.array_equal(zeros.cpu().numpy()[sel].view(np.uint32), ref["zeros"].view(np.uint32))
+    assert np.array_equal(codes.cpu().numpy()[sel], ref["codes"])
+    assert np.array_equal(acc.cpu().numpy()[sel], ref["acc"])
+    gy = bits_host(y)[sel]
+    nbad = int((gy != ref["y"]).sum())
+    assert nbad == 0, "asym bf16 output differs at %d of %d places" % (nbad, gy.size)
+
+
+def test_asym_config1():
+    L = make_layer("c1", "linear")
+    sp = L["spec"]
+    run_asym(L["x"], L, sp.alpha, sp.gamma, L["b"])
+
+
+@pytest.mark.parametrize("T,K,N,B", [(1, 128, 8, 0), (130, 384, 264, 0), (257, 1024, 520, 128),
+                                     (70, 4096, 200, 0), (33, 11008, 136, 0), (9, 28672, 64, 128)])
+def test_asym_shapes(T, K, N, B):
+    rng = np.random.default_rng(3 * T + 5 * K + 7 * N + B)
+    x = rand_x(rng, T, K, spread=1.0)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    run_asym(x, _rand_w(rng, N, K), 0.9, 1.05, b, had_block=B)
+
+
+def test_asym_degenerate_rows_and_offsets():
+    # constant rows (floor scale), all-positive rows far from zero, and alpha = 1 (no clipping)
+    rng = np.random.default_rng(41)
+    K, N = 512, 72
+    x = np.zeros((6, K), dtype=np.float32)
+    x[0] = 5.0
+    x[1] = rng.random(K) + 100.0
+    x[2] = -rng.random(K) - 50.0
+    x[3] = rng.standard_normal(K)
+    x[4] = 0.0
+    x[5] = np.arange(K) % 16
+    W = _rand_w(rng, N, K, bias=False)
+    run_asym(f32_to_bf16_bits(x), W, 1.0, 1.0, None)
+    run_asym(f32_to_bf16_bits(x), W, 0.5, 1.0, None)
+
+
+def test_asym_full_size_sampled_rows():
+    L = make_layer("c3", "up")
+    sp = L["spec"]
+    rows = np.r_[0:3, 2047:2050, 4093:4096]
+    run_asym(L["x"], L, sp.alpha, sp.gamma, L["b"], rows=rows)
+
+
+def test_asym_rejects_per_channel_sa():
+    x = torch.zeros((4, 256), dtype=torch.bfloat16, device="cuda")
+    sa = torch.ones(256, device="cuda")
+    with pytest.raises(bq.BaseqError) as e:
+        bq.quantize_act_asym(x, bq.ActParams(0.9, 1.0, sa))
+    assert e.value.status == 6
