@@ -177,30 +177,48 @@ __device__ __forceinline__ uint32_t dequant_bracket(int32_t raw, float st256, fl
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));   // hi -> upper half
   return pk;
 }
-// Asymmetric variant: y* = (s_t s_w) acc + (z_t s_w) wsum + fb.  The two products are large and
-// nearly cancel (that is what a lower bound z_t far from zero means), so an fp32 evaluation's error
-// bracket is ~80x wider than |y| and almost never settles (measured: the bracketed version spent
-// most chunks in the fp64 fix-up).  The fp64 expression is therefore evaluated directly for every
-// element (5 DP operations + 2 conversions per output; B200's FP64 rate is half its FP32 rate).
-__device__ __forceinline__ uint32_t dequant_f64_asym(int32_t acc, double std_, double ztd, float sw,
-                                                     float fb, float ws) {
+// Asymmetric variant (NEXT-1): the oracle's value is yd = fma(s_t s_w, acc, fma(z_t s_w, wsum, fb))
+// in fp64 with acc = sum_k q w over the UNSIGNED codes.  Evaluated like that in fp32 the two
+// products are ~80x larger than y and nearly cancel (q = q' + 8 puts 8 s_t wsum into the first and
+// z_t ~ -8 s_t into the second), so the bracket almost never settled (measured).  The MMA therefore
+// accumulates acc' = sum_k (q - 8) w = acc - 8 wsum, and the fast path evaluates the algebraically
+// identical  y* = (s_t s_w) acc' + (mid_t s_w) wsum + fb,  mid_t = z_t + 8 s_t  (the centre of the
+// row's range; no structural cancellation):
+//   t = RN(s_t acc'), p = RN(t s_w), midf = RN(8 s_t + z_t), mw = RN(midf wsum), m = RN(mw s_w),
+//   c = RN(mw s_w + fb), y = RN(t s_w + c)
+//   |y - y*| <= 2^-24 (|p| + |y| + |c| + 2 |m|) (1 + 2^-22)      [one term per rounding above]
+// and |yd - y*| is ~2^-52 of the same magnitudes, so E = 2^-23 (|p| + |y| + |c| + 2 |m| + 2^-100)
+// is a bracket for yd; unsettled elements take the fp64 expression itself, with acc rebuilt
+// exactly as acc' + 8 wsum.
+__device__ __noinline__ uint32_t dequant_f64_asym(int32_t acc_c, float st, float zt, float sw,
+                                                  float fb, float ws) {
+  const int32_t acc = acc_c + 8 * static_cast<int32_t>(ws);
   const double swd = static_cast<double>(sw);
-  const double c = __fma_rn(__dmul_rn(ztd, swd), static_cast<double>(ws), static_cast<double>(fb));
-  const double yd = __fma_rn(__dmul_rn(std_, swd), static_cast<double>(acc), c);
+  const double c = __fma_rn(__dmul_rn(static_cast<double>(zt), swd), static_cast<double>(ws),
+                            static_cast<double>(fb));
+  const double yd = __fma_rn(__dmul_rn(static_cast<double>(st), swd), static_cast<double>(acc), c);
   return bf16_from_double_rne(yd);
 }
-// two bracket pairs -> the output word bf16(lo0) | bf16(lo1) << 16; `unsettled` collects the
-// difference between the word of the low ends and the word of the high ends
-__device__ __forceinline__ uint32_t settle2(uint32_t k0, uint32_t k1, uint32_t& unsettled) {
-  const uint32_t los = __byte_perm(k0, k1, 0x5410);
-  const uint32_t his = __byte_perm(k0, k1, 0x7632);
-  unsettled |= los ^ his;
-  return los;
+__device__ __forceinline__ uint32_t dequant_bracket_asym(int32_t raw, float st256, float midf, float sw,
+                                                         float fb, float ws) {
+  const float t = __fmul_rn(st256, __int2float_rn(raw));
+  const float p = __fmul_rn(t, sw);
+  const float mw = __fmul_rn(midf, ws);
+  const float m = __fmul_rn(mw, sw);
+  const float c = __fmaf_rn(mw, sw, fb);
+  const float y = __fmaf_rn(t, sw, c);
+  float s = __fadd_rn(__fadd_rn(fabsf(p), 7.888609052210118e-31f), fabsf(y));
+  s = __fmaf_rn(fabsf(m), 2.0f, __fadd_rn(s, fabsf(c)));
+  const float hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);
+  const float lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
+  uint32_t pk;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));
+  return pk;
 }
-
 // ------------------------------------------------------------------------------ the kernel
 // CG = 1: one CTA per tile of 128 x BN;  CG = 2: a CTA pair per tile of 256 x BN.
-// ASYM (NEXT-1): unsigned activation codes (A format U8) and the epilogue term z_t s_w wsum[n].
+// ASYM (NEXT-1): unsigned activation codes, re-centred to q - 8 while they are expanded, and the
+// epilogue term (z_t + 8 s_t) s_w wsum[n].
 template <int CG, bool FUSED, bool ASYM>
 __global__ void __launch_bounds__((Cfg<CG, FUSED>::kThreads), 1)
 w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
@@ -304,7 +322,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     // waterfall (~95 SASS instructions and ~670 clk per k-block, measured -- slower than the
     // 384 clk the four MMAs take).
     if (leader) {
-      constexpr uint32_t idesc = ptx::make_idesc_i8(BM * CG, BN, ASYM);
+      constexpr uint32_t idesc = ptx::make_idesc_i8(BM * CG, BN);
       int stage = 0, as = 0;
       uint32_t phase = 0, aphase = 0;
       const uint64_t desc0 = ptx::make_smem_desc_sw128(unpacked0);
@@ -499,10 +517,13 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           const uint4 w = w4[c];
-          r[8 * c + 0] = (w.x << 4) & 0xF0F0F0F0u; r[8 * c + 4] = w.x & 0xF0F0F0F0u;
-          r[8 * c + 1] = (w.y << 4) & 0xF0F0F0F0u; r[8 * c + 5] = w.y & 0xF0F0F0F0u;
-          r[8 * c + 2] = (w.z << 4) & 0xF0F0F0F0u; r[8 * c + 6] = w.z & 0xF0F0F0F0u;
-          r[8 * c + 3] = (w.w << 4) & 0xF0F0F0F0u; r[8 * c + 7] = w.w & 0xF0F0F0F0u;
+          // ASYM: the unsigned code q becomes the signed byte 16 (q - 8) (flip the byte's top bit;
+          // the xor folds into the same LOP3), so the MMA accumulates acc' = acc - 8 wsum
+          constexpr uint32_t kFlip = ASYM ? 0x80808080u : 0u;
+          r[8 * c + 0] = ((w.x << 4) & 0xF0F0F0F0u) ^ kFlip; r[8 * c + 4] = (w.x & 0xF0F0F0F0u) ^ kFlip;
+          r[8 * c + 1] = ((w.y << 4) & 0xF0F0F0F0u) ^ kFlip; r[8 * c + 5] = (w.y & 0xF0F0F0F0u) ^ kFlip;
+          r[8 * c + 2] = ((w.z << 4) & 0xF0F0F0F0u) ^ kFlip; r[8 * c + 6] = (w.z & 0xF0F0F0F0u) ^ kFlip;
+          r[8 * c + 3] = ((w.w << 4) & 0xF0F0F0F0u) ^ kFlip; r[8 * c + 7] = (w.w & 0xF0F0F0F0u) ^ kFlip;
         }
         ptx::mbar_wait(ptx::smem_u32(&bars->empty[us]), uphase ^ 1u);
         ptx::tcgen05_fence_after();
@@ -533,9 +554,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       const bool row_ok = row < p.T;
       const float st = row_ok ? p.scales[row] : 0.0f;
       const float st256 = __fmul_rn(st, 0.00390625f);
-      const double std_ = static_cast<double>(st);
-      const double ztd = (ASYM && row_ok) ? static_cast<double>(p.zeros[row]) : 0.0;
-      (void)std_; (void)ztd;
+      const float zt = (ASYM && row_ok) ? p.zeros[row] : 0.0f;
+      const float midf = __fmaf_rn(8.0f, st, zt);
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
       ptx::tcgen05_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN +
@@ -549,43 +569,40 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
         ptx::tmem_ld_32x32b_x16(taddr + c0, r);
         ptx::tmem_ld_wait();
         uint32_t out[8];
-        uint32_t unsettled = 0;
 #pragma unroll
         for (int j = 0; j < 16; j += 4) {
           const int n = n0 + c0 + j;
           const float4 sw = __ldg(reinterpret_cast<const float4*>(p.sw + n));
           const float4 fb = __ldg(reinterpret_cast<const float4*>(p.fb + n));
-          if (ASYM) {
-            const float4 ws = __ldg(reinterpret_cast<const float4*>(p.wsum + n));
-            const uint32_t v0 = dequant_f64_asym(static_cast<int32_t>(r[j]) >> 8, std_, ztd, sw.x, fb.x, ws.x);
-            const uint32_t v1 = dequant_f64_asym(static_cast<int32_t>(r[j + 1]) >> 8, std_, ztd, sw.y, fb.y, ws.y);
-            const uint32_t v2 = dequant_f64_asym(static_cast<int32_t>(r[j + 2]) >> 8, std_, ztd, sw.z, fb.z, ws.z);
-            const uint32_t v3 = dequant_f64_asym(static_cast<int32_t>(r[j + 3]) >> 8, std_, ztd, sw.w, fb.w, ws.w);
-            out[j >> 1] = v0 | (v1 << 16);
-            out[(j >> 1) + 1] = v2 | (v3 << 16);
-            continue;
-          }
-          const uint32_t k0 = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw.x, fb.x);
-          const uint32_t k1 = dequant_bracket(static_cast<int32_t>(r[j + 1]), st256, sw.y, fb.y);
-          const uint32_t k2 = dequant_bracket(static_cast<int32_t>(r[j + 2]), st256, sw.z, fb.z);
-          const uint32_t k3 = dequant_bracket(static_cast<int32_t>(r[j + 3]), st256, sw.w, fb.w);
-          out[j >> 1] = settle2(k0, k1, unsettled);
-          out[(j >> 1) + 1] = settle2(k2, k3, unsettled);
-        }
-        if (unsettled != 0) {
-          // rare (about 2.4e-4 of the elements): redo the chunk's unsettled elements with the fp64
-          // expression itself
+          float4 ws = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+          if (ASYM) ws = __ldg(reinterpret_cast<const float4*>(p.wsum + n));
+          const float swv[4] = {sw.x, sw.y, sw.z, sw.w}, fbv[4] = {fb.x, fb.y, fb.z, fb.w};
+          const float wsv[4] = {ws.x, ws.y, ws.z, ws.w};
+          uint32_t k[4];
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const int n = n0 + c0 + j;
-            const float sw = __ldg(p.sw + n), fb = __ldg(p.fb + n);
-            const uint32_t k = dequant_bracket(static_cast<int32_t>(r[j]), st256, sw, fb);
-            if ((k >> 16) != (k & 0xFFFFu)) {
-              const uint32_t v = dequant_f64(static_cast<int32_t>(r[j]) >> 8, st, sw, fb);
-              out[j >> 1] = (j & 1) ? ((out[j >> 1] & 0x0000FFFFu) | (v << 16))
-                                    : ((out[j >> 1] & 0xFFFF0000u) | v);
+          for (int e = 0; e < 4; ++e)
+            k[e] = ASYM ? dequant_bracket_asym(static_cast<int32_t>(r[j + e]), st256, midf, swv[e], fbv[e], wsv[e])
+                        : dequant_bracket(static_cast<int32_t>(r[j + e]), st256, swv[e], fbv[e]);
+          // words of the low ends and of the high ends of the four brackets
+          uint32_t lo01 = __byte_perm(k[0], k[1], 0x5410), lo23 = __byte_perm(k[2], k[3], 0x5410);
+          const uint32_t hi01 = __byte_perm(k[0], k[1], 0x7632), hi23 = __byte_perm(k[2], k[3], 0x7632);
+          if (((lo01 ^ hi01) | (lo23 ^ hi23)) != 0) {
+            // rare (2.4e-4 of the elements, symmetric; ~1e-3 asymmetric): some bracket of this
+            // group straddles a bf16 rounding boundary -- evaluate the fp64 expression itself for
+            // those elements (operands are still in registers)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              if ((k[e] >> 16) != (k[e] & 0xFFFFu)) {
+                const int32_t a = static_cast<int32_t>(r[j + e]) >> 8;
+                const uint32_t v = ASYM ? dequant_f64_asym(a, st, zt, swv[e], fbv[e], wsv[e])
+                                        : dequant_f64(a, st, swv[e], fbv[e]);
+                uint32_t& w = (e < 2) ? lo01 : lo23;
+                w = (e & 1) ? ((w & 0x0000FFFFu) | (v << 16)) : ((w & 0xFFFF0000u) | v);
+              }
             }
           }
+          out[j >> 1] = lo01;
+          out[(j >> 1) + 1] = lo23;
         }
         if (row_ok) {
 #pragma unroll
@@ -597,7 +614,11 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
               if (p.acc_dump != nullptr) {
                 int32_t* d = p.acc_dump + static_cast<int64_t>(row) * p.N + n;
 #pragma unroll
-                for (int e = 0; e < 8; ++e) d[e] = static_cast<int32_t>(r[8 * g + e]) >> 8;   // raw = 256 * acc
+                for (int e = 0; e < 8; ++e) {
+                  int32_t a = static_cast<int32_t>(r[8 * g + e]) >> 8;   // raw = 256 * acc
+                  if (ASYM) a += 8 * static_cast<int32_t>(__ldg(p.wsum + n + e));   // acc' -> acc
+                  d[e] = a;
+                }
               }
             }
           }
