@@ -166,15 +166,19 @@ __device__ __noinline__ uint32_t dequant_f64(int32_t acc, float st, float sw, fl
 //   hi, lo = y +- 2^-23 (|p| + |y| + 2^-100)
 // (the 2^-100 keeps the bracket wider than the absolute rounding errors when y is denormal).
 // The element is settled iff both halves are equal.
-__device__ __forceinline__ uint32_t dequant_bracket(int32_t raw, float st256, float sw, float fb) {
+__device__ __forceinline__ void dequant_bracket(int32_t raw, float st256, float sw, float fb,
+                                                float& lo, float& hi) {
   const float t = __fmul_rn(st256, __int2float_rn(raw));
   const float p = __fmul_rn(t, sw);
   const float y = __fmaf_rn(t, sw, fb);
   const float s = __fadd_rn(__fadd_rn(fabsf(p), 7.888609052210118e-31f), fabsf(y));
-  const float hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);
-  const float lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
+  hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);
+  lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
+}
+// bf16(a1) << 16 | bf16(a0), both RNE: two bracket ends of neighbouring columns -> one output word
+__device__ __forceinline__ uint32_t pack_bf16x2(float a1, float a0) {
   uint32_t pk;
-  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));   // hi -> upper half
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(a1), "f"(a0));
   return pk;
 }
 // Asymmetric variant (NEXT-1): the oracle's value is yd = fma(s_t s_w, acc, fma(z_t s_w, wsum, fb))
@@ -199,8 +203,8 @@ __device__ __noinline__ uint32_t dequant_f64_asym(int32_t acc_c, float st, float
   const double yd = __fma_rn(__dmul_rn(static_cast<double>(st), swd), static_cast<double>(acc), c);
   return bf16_from_double_rne(yd);
 }
-__device__ __forceinline__ uint32_t dequant_bracket_asym(int32_t raw, float st256, float midf, float sw,
-                                                         float fb, float ws) {
+__device__ __forceinline__ void dequant_bracket_asym(int32_t raw, float st256, float midf, float sw,
+                                                     float fb, float ws, float& lo, float& hi) {
   const float t = __fmul_rn(st256, __int2float_rn(raw));
   const float p = __fmul_rn(t, sw);
   const float mw = __fmul_rn(midf, ws);
@@ -209,12 +213,10 @@ __device__ __forceinline__ uint32_t dequant_bracket_asym(int32_t raw, float st25
   const float y = __fmaf_rn(t, sw, c);
   float s = __fadd_rn(__fadd_rn(fabsf(p), 7.888609052210118e-31f), fabsf(y));
   s = __fmaf_rn(fabsf(m), 2.0f, __fadd_rn(s, fabsf(c)));
-  const float hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);
-  const float lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
-  uint32_t pk;
-  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk) : "f"(hi), "f"(lo));
-  return pk;
+  hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);
+  lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
 }
+
 // ------------------------------------------------------------------------------ the kernel
 // CG = 1: one CTA per tile of 128 x BN;  CG = 2: a CTA pair per tile of 256 x BN.
 // ASYM (NEXT-1): unsigned activation codes, re-centred to q - 8 while they are expanded, and the
@@ -578,21 +580,23 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           if (ASYM) ws = __ldg(reinterpret_cast<const float4*>(p.wsum + n));
           const float swv[4] = {sw.x, sw.y, sw.z, sw.w}, fbv[4] = {fb.x, fb.y, fb.z, fb.w};
           const float wsv[4] = {ws.x, ws.y, ws.z, ws.w};
-          uint32_t k[4];
+          float lo[4], hi[4];
 #pragma unroll
-          for (int e = 0; e < 4; ++e)
-            k[e] = ASYM ? dequant_bracket_asym(static_cast<int32_t>(r[j + e]), st256, midf, swv[e], fbv[e], wsv[e])
-                        : dequant_bracket(static_cast<int32_t>(r[j + e]), st256, swv[e], fbv[e]);
-          // words of the low ends and of the high ends of the four brackets
-          uint32_t lo01 = __byte_perm(k[0], k[1], 0x5410), lo23 = __byte_perm(k[2], k[3], 0x5410);
-          const uint32_t hi01 = __byte_perm(k[0], k[1], 0x7632), hi23 = __byte_perm(k[2], k[3], 0x7632);
-          if (((lo01 ^ hi01) | (lo23 ^ hi23)) != 0) {
+          for (int e = 0; e < 4; ++e) {
+            if (ASYM) dequant_bracket_asym(static_cast<int32_t>(r[j + e]), st256, midf, swv[e], fbv[e], wsv[e], lo[e], hi[e]);
+            else dequant_bracket(static_cast<int32_t>(r[j + e]), st256, swv[e], fbv[e], lo[e], hi[e]);
+          }
+          // output words of the low ends and of the high ends of the four brackets
+          uint32_t lo01 = pack_bf16x2(lo[1], lo[0]), lo23 = pack_bf16x2(lo[3], lo[2]);
+          const uint32_t d01 = lo01 ^ pack_bf16x2(hi[1], hi[0]), d23 = lo23 ^ pack_bf16x2(hi[3], hi[2]);
+          if ((d01 | d23) != 0) {
             // rare (2.4e-4 of the elements, symmetric; ~1e-3 asymmetric): some bracket of this
             // group straddles a bf16 rounding boundary -- evaluate the fp64 expression itself for
             // those elements (operands are still in registers)
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-              if ((k[e] >> 16) != (k[e] & 0xFFFFu)) {
+              const uint32_t d = (e < 2) ? d01 : d23;
+              if (((e & 1) ? (d >> 16) : (d & 0xFFFFu)) != 0) {
                 const int32_t a = static_cast<int32_t>(r[j + e]) >> 8;
                 const uint32_t v = ASYM ? dequant_f64_asym(a, st, zt, swv[e], fbv[e], wsv[e])
                                         : dequant_f64(a, st, swv[e], fbv[e]);
