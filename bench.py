@@ -300,6 +300,7 @@ def run_gpu(args):
 
     # ---- the fused variant (a10) on the same layers, reported beside the two-kernel path
     fused = run_fused(args, bq, torch, plan, acts, layers, T)
+    asym = run_asym(args, bq, torch, plan, acts, layers, T)
 
     # ---- end-to-end: HOST buffers through baseq_linear_host (H2D of X and D2H of Y timed)
     e2e = run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank)
@@ -310,7 +311,8 @@ def run_gpu(args):
             "dtype": "int4xint4->int32 (tcgen05 kind::i8); fp32 quantizer; bf16 out",
             "data": "synthetic", "config": workload_config(config), "clocks": clocks,
             "e2e": e2e, "gpu_launches": nk * args.steps, "roofline": roofline,
-            "roofline_quantizer": roofline_q, "kernels": per_layer, "fused_variant": fused}
+            "roofline_quantizer": roofline_q, "kernels": per_layer, "fused_variant": fused,
+            "asym_variant": asym}
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(config, data, plan, layers, torch)
     if rank == 0:
@@ -342,6 +344,42 @@ def run_fused(args, bq, torch, plan, acts, layers, T):
                         "same_bits_as_two_kernel_path": bool(torch.equal(
                             y.view(torch.int16), L["y"].view(torch.int16)))})
     return out
+
+
+def run_asym(args, bq, torch, plan, acts, layers, T):
+    """the same step with per-token asymmetric int4 activations
+    (baseq_quantize_act_asym + baseq_w4a4_gemm_asym), device-resident, CUDA-event timed."""
+    steps = max(3, min(args.steps, 50))
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps
+
+    out, total = [], 0.0
+    for act, specs in plan:
+        a = acts[act]
+        ms = timed(lambda: bq.quantize_act_asym(a["x"], a["params"]))
+        total += ms
+        out.append({"kind": "quant_asym", "name": act, "ms": ms,
+                    "GB_per_s": 2.5 * T * a["K"] / (ms * 1e-3) / 1e9})
+        codes, scales, zeros = bq.quantize_act_asym(a["x"], a["params"])
+        for sp in specs:
+            L = layers[sp.name]
+            y = torch.empty_like(L["y"])
+            ms = timed(lambda: bq.w4a4_gemm_asym(codes, scales, zeros, L["pw"], y))
+            total += ms
+            out.append({"kind": "gemm_asym", "name": sp.name, "ms": ms,
+                        "TOP_per_s": 2.0 * T * sp.N * sp.K / (ms * 1e-3) / 1e12})
+    return {"kernels": out, "ms_per_step": total, "tokens_per_s": T / (total * 1e-3),
+            "note": "each kernel timed alone (warm L2 for the quantiser input at small K)"}
 
 
 def run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank):
