@@ -69,6 +69,8 @@ constexpr int kAStageBytes = BM * BK;   // fused variant: int8 A operand stage i
 // the MMA takes both operands from shared memory (.ss form).
 template <int CG, bool FUSED>
 struct Cfg {
+  // per-tile column operands of the epilogue (s_w, fb, wsum), one copy per accumulator stage
+  static constexpr int kColParamBytes = kAccStages * 3 * BN * 4;
   static constexpr int kEpiWarps = FUSED ? 4 : 8;           // x 32 rows; 2 column halves when 8
   static constexpr int kSets = FUSED ? 1 : kSetsMax;
   static constexpr int kAWarp0 = kEpiWarp0 + kEpiWarps;     // 8 A warps in both variants
@@ -86,7 +88,7 @@ struct Cfg {
   static constexpr int kTemptyCount = CG * kEpiWarps;
   static constexpr int kPStages = CG == 2 ? kPStagesMax : 5;
   static constexpr int kSmemBytes =
-      1024 + kAOperand + kStages * kUnpackedStage + kPStages * kPackedStage + 256;
+      1024 + kAOperand + kStages * kUnpackedStage + kPStages * kPackedStage + 256 + kColParamBytes;
   static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
 };
 
@@ -546,6 +548,30 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
     // of the tile's BN columns.  16 columns per tcgen05.ld keep the register footprint small.
     const int q = warp & 3;
     const int half = (warp - kEpiWarp0) >> 2;
+    // The tile's column operands are staged in shared memory by the epilogue threads themselves:
+    // fetched one tile ahead into registers (latency hidden behind the previous tile), published
+    // before the accumulator wait, read back with broadcast LDS.128 -- no global-load latency
+    // inside the chunk loop (r1h capture: 44 % of the epilogue warps' time).  Reuse of a stage's
+    // copy is ordered by the per-tile named barrier (a warp arrives at tile i's barrier only after
+    // it finished tile i-1, so nobody still reads the copy of tile i-2).
+    constexpr int kEpiThreads = kEpiWarps * 32;
+    constexpr int kPer = (BN + kEpiThreads - 1) / kEpiThreads;
+    float* colp = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + 256);
+    const int et = static_cast<int>(threadIdx.x) - kEpiWarp0 * 32;
+    float pre[kPer][3];
+    auto fetch = [&](int tile) {
+      const int nb = (tile / p.num_m) * BN;
+#pragma unroll
+      for (int i = 0; i < kPer; ++i) {
+        const int c = et + i * kEpiThreads;
+        if (c < BN) {
+          pre[i][0] = __ldg(p.sw + nb + c);
+          pre[i][1] = __ldg(p.fb + nb + c);
+          pre[i][2] = ASYM ? __ldg(p.wsum + nb + c) : 0.0f;
+        }
+      }
+    };
+    if (first_tile < num_tiles) fetch(first_tile);
     constexpr int kColsPerWarp = BN / (kEpiWarps / 4);
     const uint32_t tempty_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->tempty[0]), 0);
     int as = 0;
@@ -558,6 +584,19 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       const float st256 = __fmul_rn(st, 0.00390625f);
       const float zt = (ASYM && row_ok) ? p.zeros[row] : 0.0f;
       const float midf = __fmaf_rn(8.0f, st, zt);
+      float* cs = colp + as * 3 * BN;
+#pragma unroll
+      for (int i = 0; i < kPer; ++i) {
+        const int c = et + i * kEpiThreads;
+        if (c < BN) {
+          cs[c] = pre[i][0];
+          cs[BN + c] = pre[i][1];
+          if (ASYM) cs[2 * BN + c] = pre[i][2];
+        }
+      }
+      ptx::bar_sync(1, kEpiThreads);
+      if (tile + tile_step < num_tiles) fetch(tile + tile_step);
+      cs += half * kColsPerWarp;
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
       ptx::tcgen05_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN +
@@ -573,11 +612,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
         uint32_t out[8];
 #pragma unroll
         for (int j = 0; j < 16; j += 4) {
-          const int n = n0 + c0 + j;
-          const float4 sw = __ldg(reinterpret_cast<const float4*>(p.sw + n));
-          const float4 fb = __ldg(reinterpret_cast<const float4*>(p.fb + n));
+          const float4 sw = *reinterpret_cast<const float4*>(cs + c0 + j);
+          const float4 fb = *reinterpret_cast<const float4*>(cs + BN + c0 + j);
           float4 ws = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-          if (ASYM) ws = __ldg(reinterpret_cast<const float4*>(p.wsum + n));
+          if (ASYM) ws = *reinterpret_cast<const float4*>(cs + 2 * BN + c0 + j);
           const float swv[4] = {sw.x, sw.y, sw.z, sw.w}, fbv[4] = {fb.x, fb.y, fb.z, fb.w};
           const float wsv[4] = {ws.x, ws.y, ws.z, ws.w};
           float lo[4], hi[4];
