@@ -603,15 +603,11 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
                              half * kColsPerWarp;
       const int n0 = n_blk * BN + half * kColsPerWarp;
       uint16_t* yrow = p.y + static_cast<int64_t>(row) * p.ldy;
-#pragma unroll 1
-      for (int c0 = 0; c0 < kColsPerWarp; c0 += 16) {
-        if (n0 + c0 >= p.N) break;                      // warp-uniform
-        uint32_t r[16];
-        ptx::tmem_ld_32x32b_x16(taddr + c0, r);
-        ptx::tmem_ld_wait();
-        uint32_t out[8];
+      // 8 columns: two groups of 4 -> one 16-byte store per row
+      auto process8 = [&](const uint32_t (&r)[8], int c0) {
+        uint32_t out[4];
 #pragma unroll
-        for (int j = 0; j < 16; j += 4) {
+        for (int j = 0; j < 8; j += 4) {
           const float4 sw = *reinterpret_cast<const float4*>(cs + c0 + j);
           const float4 fb = *reinterpret_cast<const float4*>(cs + BN + c0 + j);
           float4 ws = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
@@ -646,26 +642,36 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           out[j >> 1] = lo01;
           out[(j >> 1) + 1] = lo23;
         }
-        if (row_ok) {
+        const int n = n0 + c0;
+        if (row_ok && n < p.N) {
+          *reinterpret_cast<uint4*>(yrow + n) = make_uint4(out[0], out[1], out[2], out[3]);
+          if (p.acc_dump != nullptr) {
+            int32_t* d = p.acc_dump + static_cast<int64_t>(row) * p.N + n;
 #pragma unroll
-          for (int g = 0; g < 2; ++g) {
-            const int n = n0 + c0 + g * 8;
-            if (n < p.N) {
-              *reinterpret_cast<uint4*>(yrow + n) =
-                  make_uint4(out[4 * g], out[4 * g + 1], out[4 * g + 2], out[4 * g + 3]);
-              if (p.acc_dump != nullptr) {
-                int32_t* d = p.acc_dump + static_cast<int64_t>(row) * p.N + n;
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                  int32_t a = static_cast<int32_t>(r[8 * g + e]) >> 8;   // raw = 256 * acc
-                  if (ASYM) a += 8 * static_cast<int32_t>(__ldg(p.wsum + n + e));   // acc' -> acc
-                  d[e] = a;
-                }
-              }
+            for (int e = 0; e < 8; ++e) {
+              int32_t a = static_cast<int32_t>(r[e]) >> 8;                      // raw = 256 * acc
+              if (ASYM) a += 8 * static_cast<int32_t>(__ldg(p.wsum + n + e));   // acc' -> acc
+              d[e] = a;
             }
           }
         }
+      };
+      // double-buffered TMEM reads: the load of the next 8 columns is in flight while these 8 are
+      // converted
+      static_assert(kColsPerWarp % 16 == 0, "chunk pairs");
+      uint32_t ra[8], rb[8];
+      ptx::tmem_ld_32x32b_x8(taddr, ra);
+#pragma unroll 1
+      for (int c0 = 0; c0 < kColsPerWarp; c0 += 16) {
+        if (n0 + c0 >= p.N) break;                      // warp-uniform
+        ptx::tmem_ld_wait_for(ra);
+        ptx::tmem_ld_32x32b_x8(taddr + c0 + 8, rb);
+        process8(ra, c0);
+        ptx::tmem_ld_wait_for(rb);
+        if (c0 + 16 < kColsPerWarp) ptx::tmem_ld_32x32b_x8(taddr + c0 + 16, ra);
+        process8(rb, c0 + 8);
       }
+      ptx::tmem_ld_wait();
       // all TMEM reads of this warp are complete (wait::ld above): release the accumulator
       ptx::tcgen05_fence_before();
       __syncwarp();
