@@ -71,6 +71,12 @@ template <int CG, bool FUSED>
 struct Cfg {
   // per-tile column operands of the epilogue (s_w, fb, wsum), one copy per accumulator stage
   static constexpr int kColParamBytes = kAccStages * 3 * BN * 4;
+  // [barriers 256 | column operands | pad] then, unfused only, the Y staging tiles of the TMA-store
+  // epilogue: per epilogue warp 32 rows x BN/2 columns of bf16 as 3 boxes of 32 rows x 64 bytes
+  static constexpr int kTailBytes = (256 + kColParamBytes + 1023) / 1024 * 1024;
+  static constexpr bool kTmaStore = !FUSED;
+  static constexpr int kStoreWarpBytes = 32 * (BN / 2) * 2;
+  static constexpr int kStoreBytes = kTmaStore ? (FUSED ? 4 : 8) * kStoreWarpBytes : 0;
   static constexpr int kEpiWarps = FUSED ? 4 : 8;           // x 32 rows; 2 column halves when 8
   static constexpr int kSets = FUSED ? 1 : kSetsMax;
   static constexpr int kAWarp0 = kEpiWarp0 + kEpiWarps;     // 8 A warps in both variants
@@ -88,7 +94,7 @@ struct Cfg {
   static constexpr int kTemptyCount = CG * kEpiWarps;
   static constexpr int kPStages = CG == 2 ? kPStagesMax : 5;
   static constexpr int kSmemBytes =
-      1024 + kAOperand + kStages * kUnpackedStage + kPStages * kPackedStage + 256 + kColParamBytes;
+      1024 + kAOperand + kStages * kUnpackedStage + kPStages * kPackedStage + kTailBytes + kStoreBytes;
   static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
 };
 
@@ -225,7 +231,8 @@ __device__ __forceinline__ void dequant_bracket_asym(int32_t raw, float st256, f
 // epilogue term (z_t + 8 s_t) s_w wsum[n].
 template <int CG, bool FUSED, bool ASYM>
 __global__ void __launch_bounds__((Cfg<CG, FUSED>::kThreads), 1)
-w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
+w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_y,
+                 const GemmParams p) {
   using C = Cfg<CG, FUSED>;
   constexpr int kEpiWarps = C::kEpiWarps;
   constexpr int kSets = C::kSets;
@@ -252,6 +259,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
 
   if (warp == kProducerWarp && lane == 0) {
     if (!FUSED) ptx::prefetch_tensormap(&tmap_a);
+    if (C::kTmaStore) ptx::prefetch_tensormap(&tmap_y);
     for (int i = 0; i < C::kPStages; ++i) {
       ptx::mbar_init(ptx::smem_u32(&bars->pfull[i]), C::kPFullCount);
       ptx::mbar_init(ptx::smem_u32(&bars->pempty[i]), C::kPEmptyCount);
@@ -572,6 +580,15 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       }
     };
     if (first_tile < num_tiles) fetch(first_tile);
+    // TMA-store epilogue (unfused): this warp's 32 x 96 bf16 block is staged in shared memory in the
+    // SWIZZLE_64B layout of three 32-row x 64-byte boxes (lane = row, conflict-free STS.128) and
+    // written by three bulk tensor stores -- a per-lane STG.128 touches 32 different 128-byte lines
+    // (32 L1 tag cycles per instruction: 20 % of the LSU pipe's load in the r1h capture); TMA also
+    // clips rows >= T and columns >= N.
+    const uint32_t stage_y = ptx::smem_u32(bars) + C::kTailBytes + (warp - kEpiWarp0) * C::kStoreWarpBytes;
+    const uint32_t stage_lane = stage_y + lane * 64;
+    const uint32_t stage_sw = (lane >> 1) & 3;
+    (void)stage_lane; (void)stage_sw;
     constexpr int kColsPerWarp = BN / (kEpiWarps / 4);
     const uint32_t tempty_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->tempty[0]), 0);
     int as = 0;
@@ -597,6 +614,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
       ptx::bar_sync(1, kEpiThreads);
       if (tile + tile_step < num_tiles) fetch(tile + tile_step);
       cs += half * kColsPerWarp;
+      if (C::kTmaStore) {
+        if (lane == 0) ptx::bulk_wait_group_read<0>();   // the previous tile's stores have read the staging tile
+        __syncwarp();
+      }
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
       ptx::tcgen05_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN +
@@ -643,8 +664,13 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
           out[(j >> 1) + 1] = lo23;
         }
         const int n = n0 + c0;
+        if (C::kTmaStore) {
+          const uint32_t dst = stage_lane + ((c0 >> 5) << 11) + ((((c0 >> 3) & 3) ^ stage_sw) << 4);
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(out[0]), "r"(out[1]),
+                       "r"(out[2]), "r"(out[3]) : "memory");
+        }
         if (row_ok && n < p.N) {
-          *reinterpret_cast<uint4*>(yrow + n) = make_uint4(out[0], out[1], out[2], out[3]);
+          if (!C::kTmaStore) *reinterpret_cast<uint4*>(yrow + n) = make_uint4(out[0], out[1], out[2], out[3]);
           if (p.acc_dump != nullptr) {
             int32_t* d = p.acc_dump + static_cast<int64_t>(row) * p.N + n;
 #pragma unroll
@@ -672,6 +698,17 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
         process8(rb, c0 + 8);
       }
       ptx::tmem_ld_wait();
+      if (C::kTmaStore) {
+        ptx::fence_proxy_async_smem();                  // this lane's STS -> visible to the TMA engine
+        __syncwarp();
+        const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM + q * 32;
+        if (lane == 0 && row0 < p.T) {
+#pragma unroll
+          for (int bx = 0; bx < kColsPerWarp / 32; ++bx)
+            if (n0 + bx * 32 < p.N) ptx::tma_store_2d(&tmap_y, stage_y + bx * 2048, n0 + bx * 32, row0);
+          ptx::bulk_commit_group();
+        }
+      }
       // all TMEM reads of this warp are complete (wait::ld above): release the accumulator
       ptx::tcgen05_fence_before();
       __syncwarp();
@@ -681,6 +718,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p)
   }
 
   // ---- teardown: nobody leaves while the peer may still touch this CTA's barriers / smem
+  if (C::kTmaStore && warp >= kEpiWarp0 && warp < kEpiWarp0 + kEpiWarps && lane == 0)
+    ptx::bulk_wait_group<0>();                          // Y stores complete before the CTA exits
   ptx::tcgen05_fence_before();
   __syncthreads();
   if (CG == 2) ptx::cluster_sync_all();
@@ -717,7 +756,7 @@ EncodeTiledFn get_encode_fn() {
 }
 
 template <int CG, bool FUSED, bool ASYM>
-cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sms,
+cudaError_t launch_cg(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, const GemmParams& p, int num_sms,
                       cudaStream_t stream) {
   using C = Cfg<CG, FUSED>;
   static bool attr_set = false;
@@ -742,7 +781,7 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const GemmParams& p, int num_sm
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG, FUSED, ASYM>, tmap_a, p);
+  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG, FUSED, ASYM>, tmap_a, tmap_y, p);
 }
 
 }  // namespace
@@ -769,6 +808,20 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
                               const_cast<uint8_t*>(g.codes), dims, strides, box, estr,
                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  }
+  // Y (unfused): bf16 [T, ldy]; box = 32 columns (64 bytes) x 32 rows, SWIZZLE_64B; the store clips
+  // rows >= T and columns >= N.
+  CUtensorMap tmap_y{};
+  if (!fused) {
+    EncodeTiledFn encode = get_encode_fn();
+    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(g.N), static_cast<cuuint64_t>(g.T)};
+    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(g.ldy) * 2};
+    const cuuint32_t box[2] = {32, 32};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(&tmap_y, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, g.y, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
   }
 
@@ -798,10 +851,10 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
     p.had_scale = g.had_scale;
     p.codes_dump = reinterpret_cast<uint32_t*>(g.codes_dump);
     if (g.zeros != nullptr) return cudaErrorNotSupported;   // fused + asymmetric: not built
-    return launch_cg<2, true, false>(tmap_a, p, g.num_sms, g.stream);
+    return launch_cg<2, true, false>(tmap_a, tmap_y, p, g.num_sms, g.stream);
   }
-  if (g.zeros != nullptr) return launch_cg<2, false, true>(tmap_a, p, g.num_sms, g.stream);
-  return launch_cg<2, false, false>(tmap_a, p, g.num_sms, g.stream);
+  if (g.zeros != nullptr) return launch_cg<2, false, true>(tmap_a, tmap_y, p, g.num_sms, g.stream);
+  return launch_cg<2, false, false>(tmap_a, tmap_y, p, g.num_sms, g.stream);
 }
 
 }  // namespace baseq
