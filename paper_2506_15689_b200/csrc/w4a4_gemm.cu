@@ -335,47 +335,67 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     // 384 clk the four MMAs take).
     if (leader) {
       constexpr uint32_t idesc = ptx::make_idesc_i8(BM * CG, BN);
-      int stage = 0, as = 0;
+      int as = 0;
       uint32_t phase = 0, aphase = 0;
       const uint64_t desc0 = ptx::make_smem_desc_sw128(unpacked0);
       const uint64_t adesc0 = ptx::make_smem_desc_sw128(aop0);
       (void)adesc0;
-      for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-        ptx::mbar_wait(ptx::smem_u32(&bars->tempty[as]), aphase ^ 1u);
+      // Flat k-block index over all of this CTA pair's tiles, unrolled over the kStages operand
+      // stages: the stage index is a compile-time constant, so the barrier addresses, the TMEM
+      // column of A and the descriptor of B are constants off loop-invariant bases (r1i capture:
+      // the issuing warp spent ~60 % of a k-block period executing a 52-instruction loop body,
+      // eight of them R2UR moves of per-stage values -- close to the 384 clk the MMAs take).
+      int kb = 0;
+      uint32_t tmem_d = tmem_base;
+      if (n_it > 0) {
+        ptx::mbar_wait(ptx::smem_u32(&bars->tempty[0]), 1u);
         ptx::tcgen05_fence_after();
-        const uint32_t tmem_d = tmem_base + as * BN;
-        for (int kb = 0; kb < p.num_kb; ++kb) {
-          ptx::mbar_wait(ptx::smem_u32(&bars->full[stage]), phase);
-          ptx::tcgen05_fence_after();
-          if (ptx::elect_one()) {
-            const uint32_t a_col = tmem_base + kACol0 + stage * (BK / 4);
-            // descriptor start-address field is in 16-byte units: + stage bytes/16, + 2 per K chunk
-            const uint64_t db = desc0 + static_cast<uint64_t>(stage * (C::kUnpackedStage >> 4));
+      }
+      for (int base = 0; base < n_it; base += kStages) {
 #pragma unroll
-            for (int k = 0; k < BK / 32; ++k) {
-              const uint32_t accum = (kb | k) != 0 ? 1u : 0u;
-              if (FUSED) {
-                const uint64_t da = adesc0 + static_cast<uint64_t>(stage * (kAStageBytes >> 4)) + 2 * k;
-                if (CG == 2) ptx::mma_i8_ss_2cta(tmem_d, da, db + 2 * k, idesc, accum);
-                else ptx::mma_i8_ss(tmem_d, da, db + 2 * k, idesc, accum);
-              } else {
-                if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
-                else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+        for (int stage = 0; stage < kStages; ++stage) {
+          if (base + stage < n_it) {
+            ptx::mbar_wait(ptx::smem_u32(&bars->full[stage]), phase);
+            ptx::tcgen05_fence_after();
+            if (ptx::elect_one()) {
+              const uint32_t a_col = tmem_base + kACol0 + stage * (BK / 4);
+              // descriptor start-address field is in 16-byte units: + stage bytes/16, + 2 per K chunk
+              const uint64_t db = desc0 + static_cast<uint64_t>(stage * (C::kUnpackedStage >> 4));
+#pragma unroll
+              for (int k = 0; k < BK / 32; ++k) {
+                const uint32_t accum = (k != 0 || kb != 0) ? 1u : 0u;
+                if (FUSED) {
+                  const uint64_t da = adesc0 + static_cast<uint64_t>(stage * (kAStageBytes >> 4)) + 2 * k;
+                  if (CG == 2) ptx::mma_i8_ss_2cta(tmem_d, da, db + 2 * k, idesc, accum);
+                  else ptx::mma_i8_ss(tmem_d, da, db + 2 * k, idesc, accum);
+                } else {
+                  if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+                  else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+                }
+              }
+              // frees the operand stage (A columns + B smem) in every CTA of the pair
+              if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
+              else ptx::tcgen05_commit(ptx::smem_u32(&bars->empty[stage]));
+            }
+            __syncwarp();
+            if (++kb == p.num_kb) {
+              // tile complete: publish the accumulator, move to the other accumulator stage
+              kb = 0;
+              if (ptx::elect_one()) {
+                if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->tfull[as]), 3);
+                else ptx::tcgen05_commit(ptx::smem_u32(&bars->tfull[as]));
+              }
+              __syncwarp();
+              advance(as, aphase, kAccStages);
+              tmem_d = tmem_base + as * BN;
+              if (base + stage + 1 < n_it) {
+                ptx::mbar_wait(ptx::smem_u32(&bars->tempty[as]), aphase ^ 1u);
+                ptx::tcgen05_fence_after();
               }
             }
-            // frees the operand stage (A columns + B smem) in every CTA of the pair
-            if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
-            else ptx::tcgen05_commit(ptx::smem_u32(&bars->empty[stage]));
           }
-          __syncwarp();
-          advance(stage, phase, kStages);
         }
-        if (ptx::elect_one()) {
-          if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->tfull[as]), 3);
-          else ptx::tcgen05_commit(ptx::smem_u32(&bars->tfull[as]));
-        }
-        __syncwarp();
-        advance(as, aphase, kAccStages);
+        phase ^= 1u;
       }
     }
   } else if (warp >= kUnpackWarp0 && warp < kUnpackWarp0 + kNumUnpackWarps * kSets) {
