@@ -257,7 +257,16 @@ def run_gpu(args):
         evs[k][0].record()
         step(evs[k])
     torch.cuda.synchronize()
+    in_region = len(sampler.samples)
+    # NVML calls can take tens of ms on a busy GPU: if the timed region was too short for a handful
+    # of samples, keep the same load running (untimed) until there are some
+    t_end = time.time() + 2.0
+    while sampler.ok and len(sampler.samples) < 8 and time.time() < t_end:
+        for _ in range(20):
+            step(None)
+        torch.cuda.synchronize()
     clocks = sampler.stop()
+    clocks["samples_in_timed_region"] = in_region
     if ws > 1:
         dist.barrier()
     total_ms = evs[0][0].elapsed_time(evs[-1][nk])
