@@ -285,7 +285,14 @@ def run_gpu(args):
     quant_ms = sum(per_kernel[i] for i, kd in enumerate(kernels) if kd[0] == "quant")
     quant_bytes = sum(kd[2] for kd in kernels if kd[0] == "quant")
     tops = gemm_ops / (gemm_ms * 1e-3) / 1e12
-    int8_peak = 2.0 * peaks["bf16_sustained"]
+    # The "sustained" bf16 figure was taken over 4 s at power-capped clocks (MEASURED_PEAKS.json:
+    # median 1350 MHz); this step runs for tens of ms at the full SM clock, the regime of the "burst"
+    # figure.  Use burst when the sampled clock sits at the maximum, sustained otherwise, and print
+    # the fraction of the other one and of the nominal peak beside it.
+    at_max = bool(clocks.get("sm_mhz") and clocks.get("sm_max_mhz") and
+                  clocks["sm_mhz"] >= 0.95 * clocks["sm_max_mhz"])
+    which = "burst" if at_max else "sustained"
+    int8_peak = 2.0 * peaks["bf16_" + which]
     traffic = None     # dram bytes per launch of the dominant kernel, from the ncu capture in profiles/
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
@@ -295,8 +302,12 @@ def run_gpu(args):
                 traffic = int(f[2])
     roofline = {"bound": "tensor", "kernel": "w4a4_gemm_kernel", "achieved": tops, "peak": int8_peak,
                 "unit": "TFLOP/s", "frac": tops / int8_peak, "traffic": traffic,
-                "peak_source": "2 x %s bf16 sustained (%s MEASURED_PEAKS.json; int8:bf16 nominal ratio 2)"
-                               % (peaks["bf16_sustained"], peaks["source"]),
+                "peak_source": "2 x %s bf16 %s (%s MEASURED_PEAKS.json; int8:bf16 nominal ratio 2; "
+                               "SM clock %s of %s MHz during the timed region)"
+                               % (peaks["bf16_" + which], which, peaks["source"], clocks.get("sm_mhz"),
+                                  clocks.get("sm_max_mhz")),
+                "frac_of_2x_bf16_sustained": tops / (2.0 * peaks["bf16_sustained"]),
+                "frac_of_2x_bf16_burst": tops / (2.0 * peaks["bf16_burst"]),
                 "frac_of_nominal_4500": tops / 4500.0,
                 "avg_launch_ms": gemm_ms / n_gemm, "share_of_step": gemm_ms / per_kernel.sum()}
     qgbs = quant_bytes / (quant_ms * 1e-3) / 1e9
