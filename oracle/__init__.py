@@ -18,4 +18,5 @@ from .binding import (  # noqa: F401
     gemm_i32_asym,
     epilogue_asym,
     linear_asym,
+    quantize_kv,
 )

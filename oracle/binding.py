@@ -184,6 +184,27 @@ def quantize_act_asym(x_bf16, alpha, gamma=1.0, sa=None, b=None, had_block=0):
     return codes, scales, zeros
 
 
+def quantize_kv(x_bf16, n_heads, head_dim, alpha=1.0):
+    """NEXT-3: KV-cache "per-head asymmetric dynamic quantization", heads =
+    contiguous column blocks of head_dim that never straddle groups.  Each (token, head)
+    group is quantised by the asymmetric rule of Eq. 4 on its own min / max -- i.e.
+    oracle_quantize_act_asym applied to the [T * n_heads, head_dim] view with gamma = 1, no bias.
+    Returns (codes u8 [T, n_heads*head_dim/2], scales f32 [T, n_heads], zeros f32 [T, n_heads])."""
+    _chk(x_bf16, np.uint16, "x_bf16")
+    T, HD = x_bf16.shape
+    if HD != n_heads * head_dim or head_dim % 2:
+        raise ValueError("quantize_kv: x must be [T, n_heads * head_dim]")
+    groups = np.ascontiguousarray(x_bf16).reshape(T * n_heads, head_dim)
+    codes = np.empty((T * n_heads, head_dim // 2), dtype=np.uint8)
+    scales = np.empty((T * n_heads,), dtype=np.float32)
+    zeros = np.empty((T * n_heads,), dtype=np.float32)
+    rc = _load().oracle_quantize_act_asym(_ptr(groups), head_dim, T * n_heads, head_dim, alpha, 1.0,
+                                          None, None, 0, _ptr(codes), _ptr(scales), _ptr(zeros))
+    if rc:
+        raise ValueError("oracle_quantize_act_asym (kv view): invalid arguments (status %d)" % rc)
+    return (codes.reshape(T, HD // 2), scales.reshape(T, n_heads), zeros.reshape(T, n_heads))
+
+
 def gemm_i32_asym(codes, w_nibbles):
     """Unsigned activation codes x signed weights.  Returns (acc [T,N] i32, wsum [N] i32)."""
     _chk(codes, np.uint8, "codes")

@@ -553,3 +553,40 @@ def test_asym_gemm_and_epilogue_identity():
                         + Fraction(float(z[t]))) for k in range(K)) + Fraction(float(fb[n]))
             assert Fraction(float(y64[t, n])) == exact          # powers of two: no rounding at all
             assert y[t, n] == oracle.bf16_from_double(float(exact))
+
+
+# =========================================================================== NEXT-3: KV cache
+def test_kv_groups_are_heads_and_do_not_straddle():
+    # contiguous blocks of head_dim; a head's codes / scale / zero depend on that head only
+    rng = np.random.default_rng(9)
+    T, H, D = 5, 4, 64
+    x = rng.standard_normal((T, H * D)).astype(np.float32)
+    c0, s0, z0 = oracle.quantize_kv(bf16(x), H, D, 1.0)
+    x2 = x.copy()
+    x2[:, 2 * D:3 * D] = 37.0 * rng.standard_normal((T, D)).astype(np.float32)   # disturb head 2 only
+    c1, s1, z1 = oracle.quantize_kv(bf16(x2), H, D, 1.0)
+    for h in (0, 1, 3):
+        assert np.array_equal(c0[:, h * D // 2:(h + 1) * D // 2], c1[:, h * D // 2:(h + 1) * D // 2])
+        assert np.array_equal(s0[:, h], s1[:, h]) and np.array_equal(z0[:, h], z1[:, h])
+    assert not np.array_equal(s0[:, 2], s1[:, 2])
+
+
+def test_kv_lattice_heads_exact_and_reconstruct():
+    # each head a shifted integer lattice (S:227 per group): head h holds h*3 - 4 + (0..15)
+    T, H, D = 3, 4, 64
+    base = np.tile(np.arange(16, dtype=np.float32), D // 16)
+    x = np.concatenate([base + (3.0 * h - 4.0) for h in range(H)])[None, :].repeat(T, axis=0)
+    c, s, z = oracle.quantize_kv(bf16(x), H, D, 1.0)
+    assert np.all(s == 1.0)
+    assert np.array_equal(z, np.tile(3.0 * np.arange(H, dtype=np.float32) - 4.0, (T, 1)))
+    assert np.array_equal(ucodes(c), np.tile(np.tile(base, H), (T, 1)).astype(np.int64))
+    # random data: per-head reconstruction error <= half a step of THAT head (alpha = 1)
+    rng = np.random.default_rng(10)
+    xr = (rng.standard_normal((6, H * D)) * np.repeat([0.1, 1.0, 10.0, 100.0], D)).astype(np.float32)
+    xb = bf16(xr)
+    xf = (xb.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+    c, s, z = oracle.quantize_kv(xb, H, D, 1.0)
+    rec = np.repeat(s, D, axis=1).astype(np.float64) * ucodes(c) + np.repeat(z, D, axis=1)
+    assert np.all(np.abs(rec - xf) <= 0.5 * np.repeat(s, D, axis=1) * (1 + 2.0 ** -18))
+    # and the steps really are per head: they follow the heads' spreads
+    assert np.all(s[:, 0] < s[:, 1]) and np.all(s[:, 1] < s[:, 2]) and np.all(s[:, 2] < s[:, 3])
