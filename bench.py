@@ -321,6 +321,7 @@ def run_gpu(args):
     # ---- the fused variant (a10) on the same layers, reported beside the two-kernel path
     fused = run_fused(args, bq, torch, plan, acts, layers, T)
     asym = run_asym(args, bq, torch, plan, acts, layers, T)
+    kv = run_kv(args, bq, torch, T, peaks["hbm_gbs"])
 
     # ---- end-to-end: HOST buffers through baseq_linear_host (H2D of X and D2H of Y timed)
     e2e = run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank)
@@ -332,7 +333,7 @@ def run_gpu(args):
             "data": "synthetic", "config": workload_config(config), "clocks": clocks,
             "e2e": e2e, "gpu_launches": nk * args.steps, "roofline": roofline,
             "roofline_quantizer": roofline_q, "kernels": per_layer, "fused_variant": fused,
-            "asym_variant": asym}
+            "asym_variant": asym, "kv_quantizer": kv}
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(config, data, plan, layers, torch)
     if rank == 0:
@@ -400,6 +401,35 @@ def run_asym(args, bq, torch, plan, acts, layers, T):
                         "TOP_per_s": 2.0 * T * sp.N * sp.K / (ms * 1e-3) / 1e12})
     return {"kernels": out, "ms_per_step": total, "tokens_per_s": T / (total * 1e-3),
             "note": "each kernel timed alone (warm L2 for the quantiser input at small K)"}
+
+
+def run_kv(args, bq, torch, T, hbm_gbs):
+    """KV-cache per-head asymmetric int4 quantiser (baseq_quantize_kv) on the K
+    (or V) tensor of a T-token prefill, cold: the launches rotate over buffer sets > 2 x L2."""
+    steps = max(10, min(args.steps, 50))
+    out = []
+    for name, H, D in (("llama-2-7b K/V: 32 heads x 128", 32, 128), ("llama-3-8b K/V: 8 heads x 128", 8, 128)):
+        by = T * H * D * 2.5 + T * H * 8.0          # bf16 in, int4 out, (scale, zero) per group
+        nbuf = int(280e6 // by) + 2
+        g = torch.Generator(device="cuda").manual_seed(1234 + H)
+        xs = [torch.randn((T, H * D), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+              for _ in range(nbuf)]
+        outs = [bq.quantize_kv(x, H, D, 0.9) for x in xs]
+        for i in range(min(nbuf, 5)):
+            bq.quantize_kv(xs[i], H, D, 0.9, *outs[i])
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(steps):
+            bq.quantize_kv(xs[k % nbuf], H, D, 0.9, *outs[k % nbuf])
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        gbs = by / (ms * 1e-3) / 1e9
+        out.append({"shape": name, "T": T, "ms": ms, "GB_per_s": gbs, "frac_of_measured_hbm": gbs / hbm_gbs,
+                    "bytes_per_element": 2.5, "buffers_rotated": nbuf})
+        del xs, outs
+    return out
 
 
 def run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank):

@@ -133,6 +133,20 @@ BASEQ_API baseq_status_t baseq_w4a4_gemm_asym(const uint8_t* codes, const float*
                                     const float* zeros, const void* packed_w, int T, int N, int K,
                                     void* y_bf16, int64_t ldy, int32_t* acc_dump, void* stream);
 
+/* ---- NEXT-3: KV-cache "per-head asymmetric dynamic quantization".  A group is one
+ * (token, head) block of head_dim contiguous channels (heads never straddle groups); every
+ * group is quantised on its own min / max by the asymmetric rule above (Eq. 4) with
+ * u = x (no gamma, bias or Hadamard):
+ *   s = max((alpha * (mx - mn)) / 15, 1e-12);  z = alpha * mn;  q = clamp(rne((x - z) * (1 / s)), 0, 15)
+ *   x_bf16 [T, ldx] bf16 (device), row t = n_heads blocks of head_dim, ldx >= n_heads * head_dim,
+ *          ldx % 8 == 0;  head_dim 64 or 128, else BASEQ_ERR_UNSUPPORTED
+ *   codes  [T, n_heads * head_dim / 2] u8 unsigned nibbles (low nibble = even channel), contiguous
+ *   scales, zeros [T, n_heads] fp32, contiguous
+ * All buffers are caller-owned device memory; the call only enqueues on `stream`. */
+BASEQ_API baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int T, int n_heads,
+                                           int head_dim, float alpha, uint8_t* codes, float* scales,
+                                           float* zeros, void* stream);
+
 /* ---- fused variant: quantise inside the GEMM producer; int4 codes never reach HBM ----
  * A per-token absmax pre-pass writes scales_out, then one GEMM kernel whose producer warps read
  * bf16 X tiles, apply Hadamard / scale / bias / round with the known per-token scale and write

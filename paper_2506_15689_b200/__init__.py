@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     quantize_act,
     quantize_act_asym,
     w4a4_gemm_asym,
+    quantize_kv,
     w4a4_gemm,
     EXPORTED_SYMBOLS,
 )

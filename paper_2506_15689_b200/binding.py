@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = [
     "baseq_status_string", "baseq_version", "baseq_packed_weight_bytes", "baseq_pack_weights",
     "baseq_set_fused_bias", "baseq_quantize_act", "baseq_w4a4_gemm",
     "baseq_fused_workspace_bytes", "baseq_linear_fused", "baseq_linear_host_scratch_bytes",
-    "baseq_linear_host", "baseq_quantize_act_asym", "baseq_w4a4_gemm_asym",
+    "baseq_linear_host", "baseq_quantize_act_asym", "baseq_w4a4_gemm_asym", "baseq_quantize_kv",
 ]
 
 
@@ -72,6 +72,8 @@ def lib():
         L.baseq_quantize_act_asym.argtypes = [vp, i64, i32, i32, c.POINTER(_ActParamsC), vp, vp, vp, vp]
         L.baseq_w4a4_gemm_asym.restype = i32
         L.baseq_w4a4_gemm_asym.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp]
+        L.baseq_quantize_kv.restype = i32
+        L.baseq_quantize_kv.argtypes = [vp, i64, i32, i32, i32, c.c_float, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -177,6 +179,23 @@ def w4a4_gemm_asym(codes, scales, zeros, pw, y=None, acc_dump=None):
                                       _p(y), y.stride(0), _p(acc_dump), _stream()),
            "baseq_w4a4_gemm_asym")
     return y
+
+
+def quantize_kv(x, n_heads, head_dim, alpha=1.0, codes=None, scales=None, zeros=None):
+    """NEXT-3: KV-cache per-head asymmetric int4.  x bf16 [T, >= n_heads*head_dim] (row stride free).
+    Returns (codes u8 [T, n_heads*head_dim/2], scales f32 [T, n_heads], zeros f32 [T, n_heads])."""
+    T = x.shape[0]
+    assert x.dtype == torch.bfloat16 and x.stride(1) == 1
+    hd = n_heads * head_dim
+    if codes is None:
+        codes = torch.empty((T, hd // 2), dtype=torch.uint8, device=x.device)
+    if scales is None:
+        scales = torch.empty((T, n_heads), dtype=torch.float32, device=x.device)
+    if zeros is None:
+        zeros = torch.empty((T, n_heads), dtype=torch.float32, device=x.device)
+    _check(lib().baseq_quantize_kv(_p(x), x.stride(0), T, n_heads, head_dim, alpha, _p(codes),
+                                   _p(scales), _p(zeros), _stream()), "baseq_quantize_kv")
+    return codes, scales, zeros
 
 
 def linear(x, params, pw, y=None):

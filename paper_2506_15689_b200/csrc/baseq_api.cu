@@ -244,6 +244,37 @@ baseq_status_t baseq_w4a4_gemm_asym(const uint8_t* codes, const float* scales, c
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
 }
 
+baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int T, int n_heads, int head_dim,
+                                 float alpha, uint8_t* codes, float* scales, float* zeros,
+                                 void* stream) {
+  if (x_bf16 == nullptr || codes == nullptr || scales == nullptr || zeros == nullptr)
+    return BASEQ_ERR_NULL;
+  if (T < 1 || n_heads < 1 || n_heads > 65536 || T > (1 << 24)) return BASEQ_ERR_SHAPE;
+  if (head_dim != 64 && head_dim != 128) return BASEQ_ERR_UNSUPPORTED;
+  if (!(alpha >= 1.0f / 65536.0f && alpha <= 1.0f)) return BASEQ_ERR_PARAM;
+  if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4) || !aligned(zeros, 4))
+    return BASEQ_ERR_ALIGN;
+  if (ldx < static_cast<int64_t>(n_heads) * head_dim || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;
+  int sms = 0;
+  const baseq_status_t st = device_check(&sms);
+  if (st != BASEQ_OK) return st;
+  KvLaunch q{};
+  q.x = x_bf16;
+  q.ldx = ldx;
+  q.T = T;
+  q.heads = n_heads;
+  q.head_dim = head_dim;
+  q.alpha = alpha;
+  q.codes = codes;
+  q.scales = scales;
+  q.zeros = zeros;
+  q.num_sms = sms;
+  q.stream = static_cast<cudaStream_t>(stream);
+  const cudaError_t e = launch_quantize_kv(q);
+  if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
+  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+}
+
 size_t baseq_fused_workspace_bytes(int T, int N, int K) {
   (void)N;
   (void)K;

@@ -74,6 +74,20 @@ bool quantize_ring_supported(int K);
 cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes);
 
 // ------------------------------------------------------------------ weight packer
+// ------------------------------------------------------------------ KV-cache quantiser (NEXT-3)
+struct KvLaunch {
+  const void* x;        // bf16 [T, ldx], row t = heads blocks of head_dim channels
+  int64_t ldx;
+  int T, heads, head_dim;
+  float alpha;
+  uint8_t* codes;       // [T, heads * head_dim / 2] unsigned nibbles
+  float* scales;        // [T, heads]
+  float* zeros;         // [T, heads]
+  int num_sms;
+  cudaStream_t stream;
+};
+cudaError_t launch_quantize_kv(const KvLaunch& q);   // cudaErrorNotSupported: head_dim not 64 / 128
+
 cudaError_t launch_pack_weights(const uint8_t* w_nibbles, const float* w_scale, const float* b,
                                 const float* layer_bias, int N, int K, void* blob,
                                 float* fused_bias_out, cudaStream_t stream);

@@ -85,6 +85,13 @@ def test_validation_happens_before_any_launch():
     assert f(base, 256, 4, 256, ctypes.byref(ok), base, 8, base, 8, base, 0, None, base, None,
              None) == 5                                                            # workspace
     assert L.baseq_pack_weights(base, base, None, None, 8, 128, base + 16, None, None) == 3
+    kv = L.baseq_quantize_kv
+    assert kv(None, 1024, 4, 8, 128, 1.0, base, base, base, None) == 1               # NULL
+    assert kv(base, 1024, 0, 8, 128, 1.0, base, base, base, None) == 2               # empty T
+    assert kv(base, 768, 4, 8, 96, 1.0, base, base, base, None) == 6                 # head_dim
+    assert kv(base, 1024, 4, 8, 128, 0.0, base, base, base, None) == 4               # alpha
+    assert kv(base, 512, 4, 8, 128, 1.0, base, base, base, None) == 3                # ldx < H * D
+    assert kv(base + 2, 1024, 4, 8, 128, 1.0, base, base, base, None) == 3           # misaligned x
 
 
 def test_no_cpu_fallback_without_a_device():

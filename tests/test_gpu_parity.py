@@ -430,3 +430,60 @@ def test_asym_rejects_per_channel_sa():
     with pytest.raises(bq.BaseqError) as e:
         bq.quantize_act_asym(x, bq.ActParams(0.9, 1.0, sa))
     assert e.value.status == 6
+
+
+# =========================================================================== NEXT-3: KV cache
+def run_kv(x_bits, H, D, alpha, ldx=None, rows=None):
+    """baseq_quantize_kv vs oracle.quantize_kv: codes, scales, zeros bit for bit."""
+    T = x_bits.shape[0]
+    if ldx is None:
+        xd = bf16_dev(x_bits)
+    else:                                    # row stride larger than H * D: the extra columns are junk
+        pad = np.full((T, ldx), 0x7FC0, dtype=np.uint16)          # NaNs that must never be read
+        pad[:, :H * D] = x_bits
+        xd = bf16_dev(pad)[:, :H * D]
+    codes, scales, zeros = bq.quantize_kv(xd, H, D, alpha)
+    torch.cuda.synchronize()
+    sel = np.arange(T) if rows is None else rows
+    rc, rs, rz = oracle.quantize_kv(np.ascontiguousarray(x_bits[sel]), H, D, alpha)
+    assert np.array_equal(scales.cpu().numpy()[sel].view(np.uint32), rs.view(np.uint32))
+    assert np.array_equal(zeros.cpu().numpy()[sel].view(np.uint32), rz.view(np.uint32))
+    assert np.array_equal(codes.cpu().numpy()[sel], rc)
+
+
+@pytest.mark.parametrize("T,H,D", [(1, 1, 64), (1, 1, 128), (7, 3, 128), (33, 8, 128), (130, 32, 64),
+                                   (5, 5, 64), (257, 9, 128)])
+def test_kv_shapes(T, H, D):
+    rng = np.random.default_rng(11 * T + 13 * H + D)
+    x = rand_x(rng, T, H * D, spread=1.0)
+    for alpha in (1.0, 0.9):
+        run_kv(x, H, D, alpha)
+
+
+def test_kv_strided_rows_and_degenerate_groups():
+    rng = np.random.default_rng(77)
+    T, H, D = 19, 4, 128
+    x = rand_x(rng, T, H * D, spread=1.0)
+    xf = (x.astype(np.uint32) << 16).view(np.float32).copy()
+    xf[0, :D] = 3.5                      # constant head: floor scale, z = the value, codes 0
+    xf[1, D:2 * D] = 0.0                 # all-zero head
+    xf[2, 2 * D:3 * D] = np.abs(xf[2, 2 * D:3 * D]) + 100.0     # all positive, far from zero
+    xf[3, 3 * D:] *= 1e-30               # tiny magnitudes
+    xb = (xf.view(np.uint32) >> 16).astype(np.uint16)           # truncation: still bf16 patterns
+    run_kv(xb, H, D, 1.0)
+    run_kv(xb, H, D, 0.9, ldx=H * D + 64)
+
+
+def test_kv_full_size_sampled_rows():
+    # Llama-3-8B K or V of an 8192-token prefill (8 KV heads x 128) and Llama-2-7B (32 x 128, T = 4096)
+    for T, H, D, seed in ((8192, 8, 128, 5), (4096, 32, 128, 6)):
+        rng = np.random.default_rng(seed)
+        x = rand_x(rng, T, H * D, spread=1.0)
+        rows = np.unique(np.concatenate([np.arange(4), rng.integers(0, T, 24), np.arange(T - 4, T)]))
+        run_kv(x, H, D, 0.9, rows=rows)
+
+
+def test_kv_rejects_other_head_dims():
+    x = torch.zeros((4, 96 * 2), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(bq.BaseqError):
+        bq.quantize_kv(x, 2, 96)
