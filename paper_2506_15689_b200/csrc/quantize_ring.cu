@@ -241,6 +241,157 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Split variant for short rows (K = 1024 * V, V <= 4; every K = 4096 shape of the benchmark): the
+// 16 consumer warps form four independent groups of 128 threads, and row j of a 4-row stage
+// belongs to group j (thread r' of the group owns vectors r', r' + 128, ...).  Same work per
+// thread and stage as the row-wide layout (32 elements, one reduction, two barriers), but the
+// barriers are group-local, so while one group waits for its row's s_t (shuffles, barrier, two IEEE
+// divisions, barrier: ~1 us of latency in the row-wide kernel, where all 16 warps waited together)
+// the other three keep the issue slots busy.
+constexpr int kSplitGroups = 4;
+constexpr int kGroupThreads = kConsumers / kSplitGroups;   // 128
+constexpr int kGroupWarps = kGroupThreads / 32;
+
+template <int V, bool WRITE_CODES>
+__global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(const RingParams p) {
+  constexpr int RL = kSplitGroups;
+  extern __shared__ __align__(128) uint8_t ring[];
+  __shared__ uint64_t full[kMaxStages], empty[kMaxStages];
+  __shared__ float s_part[2][RL][kGroupWarps];
+  __shared__ float2 s_scale[2][RL];
+
+  const int tid = threadIdx.x;
+  const int warp = tid >> 5, lane = tid & 31;
+  const int num_groups = (p.T + RL - 1) / RL;     // one stage = RL rows
+
+  if (tid == 0) {
+    for (int s = 0; s < p.stages; ++s) {
+      ptx::mbar_init(ptx::smem_u32(&full[s]), 1);
+      ptx::mbar_init(ptx::smem_u32(&empty[s]), kConsumerWarps);
+    }
+    ptx::fence_barrier_init();
+  }
+  __syncthreads();
+
+  if (warp == kConsumerWarps) {
+    if (lane == 0) {
+      int s = 0;
+      uint32_t ph = 0;
+      const uint32_t row_bytes = static_cast<uint32_t>(p.K) * 2u;
+      for (int g = blockIdx.x; g < num_groups; g += gridDim.x) {
+        ptx::mbar_wait(ptx::smem_u32(&empty[s]), ph ^ 1u);
+        const int row0 = g * RL;
+        const int rows = (p.T - row0) < RL ? (p.T - row0) : RL;
+        const uint32_t bar = ptx::smem_u32(&full[s]);
+        ptx::mbar_arrive_expect_tx(bar, row_bytes * rows);
+        const uint32_t dst = ptx::smem_u32(ring) + s * p.stage_bytes;
+        for (int j = 0; j < rows; ++j) {
+          ptx::bulk_load_1d(dst + j * row_bytes, p.x + static_cast<int64_t>(row0 + j) * p.row_bytes_stride,
+                            row_bytes, bar);
+        }
+        if (++s == p.stages) { s = 0; ph ^= 1u; }
+      }
+    }
+    return;
+  }
+
+  const int grp = warp / kGroupWarps;              // this thread's row inside every stage
+  const int gw = warp % kGroupWarps;
+  const int r = tid & (kGroupThreads - 1);         // vectors r, r + 128, ... of that row
+  float bb[V][8];
+#pragma unroll
+  for (int i = 0; i < V; ++i) {
+    if (p.bvec != nullptr) {
+      qm::load8_pinned(p.bvec + 8 * (r + i * kGroupThreads), bb[i]);
+    } else {
+#pragma unroll
+      for (int e = 0; e < 8; ++e) bb[i][e] = 0.0f;
+    }
+  }
+
+  int s = 0, parity = 0;
+  uint32_t ph = 0;
+  for (int g = blockIdx.x; g < num_groups; g += gridDim.x, parity ^= 1) {
+    const int row = g * RL + grp;
+    const bool row_ok = row < p.T;
+    ptx::mbar_wait(ptx::smem_u32(&full[s]), ph);
+    const uint8_t* srow = ring + s * p.stage_bytes + static_cast<size_t>(grp) * p.K * 2;
+
+    float u[V][8];
+    float m = 0.0f;
+    if (row_ok) {                                   // rows past T were not loaded
+#pragma unroll
+      for (int i = 0; i < V; ++i) {
+        const uint4 xv = *reinterpret_cast<const uint4*>(srow + (r + i * kGroupThreads) * 16);
+        float f[8];
+        qm::unpack8(xv, f);
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          u[i][e] = qm::affine(p.gamma, f[e], bb[i][e]);
+          m = fmaxf(m, fabsf(u[i][e]));
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&empty[s]));
+    if (++s == p.stages) { s = 0; ph ^= 1u; }
+    if (!row_ok) continue;                          // group-uniform: the whole group skips
+
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0) s_part[parity][grp][gw] = m;
+    named_barrier_sync(1 + grp, kGroupThreads);
+    if (gw == 0 && lane == 0) {
+      float mm = s_part[parity][grp][0];
+#pragma unroll
+      for (int w = 1; w < kGroupWarps; ++w) mm = fmaxf(mm, s_part[parity][grp][w]);
+      const float st = qm::step_size(p.alpha, mm);
+      s_scale[parity][grp] = make_float2(st, qm::reciprocal(st));
+      p.scales[row] = st;
+    }
+    named_barrier_sync(5 + grp, kGroupThreads);
+
+    if (WRITE_CODES) {
+      const float inv = s_scale[parity][grp].y;
+      uint32_t* crow = p.codes + static_cast<int64_t>(row) * p.nvec;
+#pragma unroll
+      for (int i = 0; i < V; ++i) crow[r + i * kGroupThreads] = qm::quantize_pack8(u[i], inv);
+    }
+  }
+}
+
+template <int V, bool WC>
+cudaError_t launch_ring_split(const QuantLaunch& q) {
+  RingParams p{};
+  p.x = static_cast<const uint8_t*>(q.x);
+  p.row_bytes_stride = q.ldx * 2;
+  p.T = q.T;
+  p.K = q.K;
+  p.nvec = q.K / 8;
+  p.alpha = q.alpha;
+  p.gamma = q.gamma;
+  p.bvec = q.b;
+  p.codes = reinterpret_cast<uint32_t*>(q.codes);
+  p.scales = q.scales;
+  p.stage_bytes = kSplitGroups * q.K * 2;
+  int stages = kRingSmemBudget / p.stage_bytes;
+  p.stages = stages > kMaxStages ? kMaxStages : stages;
+  if (p.stages < 2) return cudaErrorInvalidValue;
+  const int smem = p.stages * p.stage_bytes;
+  static int attr_smem = 0;
+  if (smem > attr_smem) {
+    cudaError_t e = cudaFuncSetAttribute(quantize_ring_split_kernel<V, WC>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    attr_smem = smem;
+  }
+  const int groups = (q.T + kSplitGroups - 1) / kSplitGroups;
+  const int blocks = groups < q.num_sms ? groups : q.num_sms;
+  quantize_ring_split_kernel<V, WC><<<blocks, kRingThreads, smem, q.stream>>>(p);
+  return cudaGetLastError();
+}
+
 template <int V, int RL, bool HAD, bool WC, bool RAGGED, bool ASYM>
 cudaError_t launch_ring_a(const QuantLaunch& q) {
   RingParams p{};
@@ -319,6 +470,9 @@ cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes) {
   const int nvec = q.K / 8;
   const int V = (nvec + kConsumers - 1) / kConsumers;
   const int RL = q.K <= 5120 ? 4 : (q.K <= 10240 ? 2 : 1);
+  if (!q.asym && q.had_block == 0 && q.K == 4096) {
+    return write_codes ? launch_ring_split<4, true>(q) : launch_ring_split<4, false>(q);
+  }
   if (q.had_block) {
     return write_codes ? launch_ring_hw<true, true>(q, V, RL) : launch_ring_hw<true, false>(q, V, RL);
   }
