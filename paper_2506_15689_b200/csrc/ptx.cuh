@@ -11,6 +11,16 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
 
+// Programmatic dependent launch: `launch_dependents` lets the next kernel of the stream start its
+// CTAs (and run its prologue) as soon as this grid's CTAs leave their SMs; `wait` blocks until the
+// previous grid has completed and its memory is visible -- every read of a predecessor's output
+// comes after it.
+__device__ __forceinline__ void griddep_launch_dependents() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+__device__ __forceinline__ void griddep_wait() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
 // named barrier over `nthreads` threads of the CTA (id 1..15; 0 is __syncthreads)
 __device__ __forceinline__ void bar_sync(uint32_t id, uint32_t nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");

@@ -43,6 +43,22 @@ __device__ __forceinline__ void named_barrier_sync(int id, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
+// launch with programmatic stream serialisation allowed (see ptx::griddep_wait)
+template <typename Kern>
+cudaError_t launch_pdl(Kern kern, int blocks, int threads, int smem, cudaStream_t stream, const RingParams& p) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(static_cast<unsigned>(blocks), 1, 1);
+  cfg.blockDim = dim3(static_cast<unsigned>(threads), 1, 1);
+  cfg.dynamicSmemBytes = static_cast<size_t>(smem);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, p);
+}
+
 template <int V, int RL, bool HAD, bool WRITE_CODES, bool RAGGED, bool ASYM>
 __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const RingParams p) {
   extern __shared__ __align__(128) uint8_t ring[];
@@ -64,6 +80,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
     ptx::fence_barrier_init();
   }
   __syncthreads();
+  ptx::griddep_launch_dependents();
+  ptx::griddep_wait();
 
   if (warp == kConsumerWarps) {
     // ===================================================================== producer
@@ -273,6 +291,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
     ptx::fence_barrier_init();
   }
   __syncthreads();
+  ptx::griddep_launch_dependents();
+  ptx::griddep_wait();
 
   if (warp == kConsumerWarps) {
     if (lane == 0) {
@@ -388,8 +408,7 @@ cudaError_t launch_ring_split(const QuantLaunch& q) {
   }
   const int groups = (q.T + kSplitGroups - 1) / kSplitGroups;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
-  quantize_ring_split_kernel<V, WC><<<blocks, kRingThreads, smem, q.stream>>>(p);
-  return cudaGetLastError();
+  return launch_pdl(quantize_ring_split_kernel<V, WC>, blocks, kRingThreads, smem, q.stream, p);
 }
 
 template <int V, int RL, bool HAD, bool WC, bool RAGGED, bool ASYM>
@@ -422,8 +441,7 @@ cudaError_t launch_ring_a(const QuantLaunch& q) {
   }
   const int groups = (q.T + RL - 1) / RL;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
-  quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM><<<blocks, kRingThreads, smem, q.stream>>>(p);
-  return cudaGetLastError();
+  return launch_pdl(quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM>, blocks, kRingThreads, smem, q.stream, p);
 }
 
 template <int V, int RL, bool HAD, bool WC, bool RAGGED>

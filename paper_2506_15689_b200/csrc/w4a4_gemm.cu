@@ -283,6 +283,9 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
   if (CG == 2) ptx::cluster_sync_all();       // peer barriers initialised before any remote arrive
   ptx::tcgen05_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
+  // prologue done (barriers, TMEM, tensor maps): from here on the predecessor's outputs are read
+  ptx::griddep_launch_dependents();
+  ptx::griddep_wait();
 
   const int num_tiles = p.num_m * p.num_n;
   const int first_tile = static_cast<int>(blockIdx.x) / CG;
@@ -794,13 +797,15 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, cons
   cfg.blockDim = dim3(C::kThreads, 1, 1);
   cfg.dynamicSmemBytes = C::kSmemBytes;
   cfg.stream = stream;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = CG;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG, FUSED, ASYM>, tmap_a, tmap_y, p);
 }
 
