@@ -311,7 +311,7 @@ def run_gpu(args):
                 "frac_of_nominal_4500": tops / 4500.0,
                 "avg_launch_ms": gemm_ms / n_gemm, "share_of_step": gemm_ms / per_kernel.sum()}
     qgbs = quant_bytes / (quant_ms * 1e-3) / 1e9
-    roofline_q = {"bound": "hbm", "kernel": "quantize_ring_kernel", "achieved": qgbs,
+    roofline_q = {"bound": "hbm", "kernel": "quantize_ring_split_kernel (K = 4096) / quantize_ring_kernel", "achieved": qgbs,
                   "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": qgbs / peaks["hbm_gbs"],
                   "frac_of_nominal_8000": qgbs / 8000.0, "share_of_step": quant_ms / per_kernel.sum()}
     per_layer = [{"kernel": kd[0], "name": kd[1], "ms": float(per_kernel[i]),
