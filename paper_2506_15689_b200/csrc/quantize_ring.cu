@@ -271,13 +271,15 @@ constexpr int kSplitGroups = 4;
 constexpr int kGroupThreads = kConsumers / kSplitGroups;   // 128
 constexpr int kGroupWarps = kGroupThreads / 32;
 
-template <int V, bool WRITE_CODES>
+template <int V, bool WRITE_CODES, bool ASYM>
 __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(const RingParams p) {
   constexpr int RL = kSplitGroups;
   extern __shared__ __align__(128) uint8_t ring[];
   __shared__ uint64_t full[kMaxStages], empty[kMaxStages];
   __shared__ float s_part[2][RL][kGroupWarps];
+  __shared__ float s_part2[ASYM ? 2 : 1][RL][kGroupWarps];   // asymmetric: max(-u) = -min(u)
   __shared__ float2 s_scale[2][RL];
+  __shared__ float s_zero[2][RL];
 
   const int tid = threadIdx.x;
   const int warp = tid >> 5, lane = tid & 31;
@@ -339,7 +341,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
     const uint8_t* srow = ring + s * p.stage_bytes + static_cast<size_t>(grp) * p.K * 2;
 
     float u[V][8];
-    float m = 0.0f;
+    float m = ASYM ? -3.402823466e38f : 0.0f;
+    float m2 = -3.402823466e38f;                    // asymmetric only: running max of -u
     if (row_ok) {                                   // rows past T were not loaded
 #pragma unroll
       for (int i = 0; i < V; ++i) {
@@ -349,7 +352,12 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
           u[i][e] = qm::affine(p.gamma, f[e], bb[i][e]);
-          m = fmaxf(m, fabsf(u[i][e]));
+          if (ASYM) {
+            m = fmaxf(m, u[i][e]);
+            m2 = fmaxf(m2, -u[i][e]);
+          } else {
+            m = fmaxf(m, fabsf(u[i][e]));
+          }
         }
       }
     }
@@ -359,16 +367,32 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
     if (!row_ok) continue;                          // group-uniform: the whole group skips
 
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if (lane == 0) s_part[parity][grp][gw] = m;
+    for (int o = 16; o > 0; o >>= 1) {
+      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+      if (ASYM) m2 = fmaxf(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+    }
+    if (lane == 0) {
+      s_part[parity][grp][gw] = m;
+      if (ASYM) s_part2[ASYM ? parity : 0][grp][gw] = m2;
+    }
     named_barrier_sync(1 + grp, kGroupThreads);
     if (gw == 0 && lane == 0) {
       float mm = s_part[parity][grp][0];
 #pragma unroll
       for (int w = 1; w < kGroupWarps; ++w) mm = fmaxf(mm, s_part[parity][grp][w]);
-      const float st = qm::step_size(p.alpha, mm);
+      float mm2 = -3.402823466e38f;
+      if (ASYM) {
+#pragma unroll
+        for (int w = 0; w < kGroupWarps; ++w) mm2 = fmaxf(mm2, s_part2[ASYM ? parity : 0][grp][w]);
+      }
+      const float st = ASYM ? qm::step_size_asym(p.alpha, -mm2, mm) : qm::step_size(p.alpha, mm);
       s_scale[parity][grp] = make_float2(st, qm::reciprocal(st));
       p.scales[row] = st;
+      if (ASYM) {
+        const float zt = qm::lower_bound_asym(p.alpha, -mm2);
+        s_zero[parity][grp] = zt;
+        p.zeros[row] = zt;
+      }
     }
     named_barrier_sync(5 + grp, kGroupThreads);
 
@@ -376,12 +400,15 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
       const float inv = s_scale[parity][grp].y;
       uint32_t* crow = p.codes + static_cast<int64_t>(row) * p.nvec;
 #pragma unroll
-      for (int i = 0; i < V; ++i) crow[r + i * kGroupThreads] = qm::quantize_pack8(u[i], inv);
+      for (int i = 0; i < V; ++i) {
+        crow[r + i * kGroupThreads] = ASYM ? qm::quantize_pack8_asym(u[i], s_zero[parity][grp], inv)
+                                           : qm::quantize_pack8(u[i], inv);
+      }
     }
   }
 }
 
-template <int V, bool WC>
+template <int V, bool WC, bool ASYM>
 cudaError_t launch_ring_split(const QuantLaunch& q) {
   RingParams p{};
   p.x = static_cast<const uint8_t*>(q.x);
@@ -394,6 +421,7 @@ cudaError_t launch_ring_split(const QuantLaunch& q) {
   p.bvec = q.b;
   p.codes = reinterpret_cast<uint32_t*>(q.codes);
   p.scales = q.scales;
+  p.zeros = q.zeros;
   p.stage_bytes = kSplitGroups * q.K * 2;
   int stages = kRingSmemBudget / p.stage_bytes;
   p.stages = stages > kMaxStages ? kMaxStages : stages;
@@ -401,14 +429,14 @@ cudaError_t launch_ring_split(const QuantLaunch& q) {
   const int smem = p.stages * p.stage_bytes;
   static int attr_smem = 0;
   if (smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(quantize_ring_split_kernel<V, WC>,
+    cudaError_t e = cudaFuncSetAttribute(quantize_ring_split_kernel<V, WC, ASYM>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     attr_smem = smem;
   }
   const int groups = (q.T + kSplitGroups - 1) / kSplitGroups;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
-  return launch_pdl(quantize_ring_split_kernel<V, WC>, blocks, kRingThreads, smem, q.stream, p);
+  return launch_pdl(quantize_ring_split_kernel<V, WC, ASYM>, blocks, kRingThreads, smem, q.stream, p);
 }
 
 template <int V, int RL, bool HAD, bool WC, bool RAGGED, bool ASYM>
@@ -488,8 +516,9 @@ cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes) {
   const int nvec = q.K / 8;
   const int V = (nvec + kConsumers - 1) / kConsumers;
   const int RL = q.K <= 5120 ? 4 : (q.K <= 10240 ? 2 : 1);
-  if (!q.asym && q.had_block == 0 && q.K == 4096) {
-    return write_codes ? launch_ring_split<4, true>(q) : launch_ring_split<4, false>(q);
+  if (q.had_block == 0 && q.K == 4096) {
+    if (q.asym) return write_codes ? launch_ring_split<4, true, true>(q) : cudaErrorInvalidValue;
+    return write_codes ? launch_ring_split<4, true, false>(q) : launch_ring_split<4, false, false>(q);
   }
   if (q.had_block) {
     return write_codes ? launch_ring_hw<true, true>(q, V, RL) : launch_ring_hw<true, false>(q, V, RL);
