@@ -186,8 +186,10 @@ int quant_max_k() { return 512 * kMaxV * 8; }
 
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes) {
   // long rows with the scalar s^a (every benchmark shape): bulk-TMA ring kernel; a per-channel
-  // s^a vector takes the register-resident kernel below
-  if (quantize_ring_supported(q.K) && q.sa == nullptr && q.tpr_log2_override == 0)
+  // s^a vector takes the ring's split kernel at K = 4096 and the register-resident kernel below
+  // otherwise
+  if (quantize_ring_supported(q.K) && q.tpr_log2_override == 0 &&
+      (q.sa == nullptr || quantize_ring_supports_sa(q.K, q.had_block)))
     return launch_quantize_ring(q, write_codes);
   const int nvec = q.K / 8;
   // smallest power-of-two threads-per-row (>= 32) with at most 4 vectors per thread (the fp32 row

@@ -30,6 +30,7 @@ struct RingParams {
   int T, K, nvec;
   float alpha, gamma;
   const float* bvec;
+  const float* sa;         // per-channel s^a (split kernel only), or NULL for the scalar gamma
   int had_block;
   float had_scale;
   uint32_t* codes;
@@ -271,7 +272,7 @@ constexpr int kSplitGroups = 4;
 constexpr int kGroupThreads = kConsumers / kSplitGroups;   // 128
 constexpr int kGroupWarps = kGroupThreads / 32;
 
-template <int V, bool WRITE_CODES, bool ASYM>
+template <int V, bool WRITE_CODES, bool ASYM, bool SA>
 __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(const RingParams p) {
   constexpr int RL = kSplitGroups;
   extern __shared__ __align__(128) uint8_t ring[];
@@ -332,6 +333,19 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
     }
   }
 
+  // per-channel s^a (NEXT-4): u, the bias and s^a together do not fit the register file (ptxas
+  // spilled), so this thread's V x 8 values of s^a live in shared memory behind the ring, written
+  // and read by this thread only (every group writes the same values: a benign duplicate)
+  float4* sa_s = reinterpret_cast<float4*>(ring + static_cast<size_t>(p.stages) * p.stage_bytes);
+  if (SA) {
+#pragma unroll
+    for (int i = 0; i < V; ++i) {
+      const int idx = r + i * kGroupThreads;
+      sa_s[2 * idx] = __ldg(reinterpret_cast<const float4*>(p.sa) + 2 * idx);
+      sa_s[2 * idx + 1] = __ldg(reinterpret_cast<const float4*>(p.sa) + 2 * idx + 1);
+    }
+  }
+
   int s = 0, parity = 0;
   uint32_t ph = 0;
   for (int g = blockIdx.x; g < num_groups; g += gridDim.x, parity ^= 1) {
@@ -349,9 +363,15 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
         const uint4 xv = *reinterpret_cast<const uint4*>(srow + (r + i * kGroupThreads) * 16);
         float f[8];
         qm::unpack8(xv, f);
+        float gv[8];
+        if (SA) {
+          const float4 g0 = sa_s[2 * (r + i * kGroupThreads)], g1 = sa_s[2 * (r + i * kGroupThreads) + 1];
+          gv[0] = g0.x; gv[1] = g0.y; gv[2] = g0.z; gv[3] = g0.w;
+          gv[4] = g1.x; gv[5] = g1.y; gv[6] = g1.z; gv[7] = g1.w;
+        }
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
-          u[i][e] = qm::affine(p.gamma, f[e], bb[i][e]);
+          u[i][e] = qm::affine(SA ? gv[e] : p.gamma, f[e], bb[i][e]);
           if (ASYM) {
             m = fmaxf(m, u[i][e]);
             m2 = fmaxf(m2, -u[i][e]);
@@ -408,7 +428,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
   }
 }
 
-template <int V, bool WC, bool ASYM>
+template <int V, bool WC, bool ASYM, bool SA>
 cudaError_t launch_ring_split(const QuantLaunch& q) {
   RingParams p{};
   p.x = static_cast<const uint8_t*>(q.x);
@@ -419,24 +439,26 @@ cudaError_t launch_ring_split(const QuantLaunch& q) {
   p.alpha = q.alpha;
   p.gamma = q.gamma;
   p.bvec = q.b;
+  p.sa = q.sa;
   p.codes = reinterpret_cast<uint32_t*>(q.codes);
   p.scales = q.scales;
   p.zeros = q.zeros;
   p.stage_bytes = kSplitGroups * q.K * 2;
-  int stages = kRingSmemBudget / p.stage_bytes;
+  const int sa_bytes = SA ? q.K * 4 : 0;
+  int stages = (kRingSmemBudget - sa_bytes) / p.stage_bytes;
   p.stages = stages > kMaxStages ? kMaxStages : stages;
   if (p.stages < 2) return cudaErrorInvalidValue;
-  const int smem = p.stages * p.stage_bytes;
+  const int smem = p.stages * p.stage_bytes + sa_bytes;
   static int attr_smem = 0;
   if (smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(quantize_ring_split_kernel<V, WC, ASYM>,
+    cudaError_t e = cudaFuncSetAttribute(quantize_ring_split_kernel<V, WC, ASYM, SA>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     attr_smem = smem;
   }
   const int groups = (q.T + kSplitGroups - 1) / kSplitGroups;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
-  return launch_pdl(quantize_ring_split_kernel<V, WC, ASYM>, blocks, kRingThreads, smem, q.stream, p);
+  return launch_pdl(quantize_ring_split_kernel<V, WC, ASYM, SA>, blocks, kRingThreads, smem, q.stream, p);
 }
 
 template <int V, int RL, bool HAD, bool WC, bool RAGGED, bool ASYM>
@@ -511,14 +533,22 @@ cudaError_t launch_ring_hw(const QuantLaunch& q, int V, int RL) {
 }  // namespace
 
 bool quantize_ring_supported(int K) { return K >= 4096 && K <= 32768; }
+// a per-channel s^a vector is handled by the split kernel only
+bool quantize_ring_supports_sa(int K, int had_block) { return K == 4096 && had_block == 0; }
 
 cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes) {
   const int nvec = q.K / 8;
   const int V = (nvec + kConsumers - 1) / kConsumers;
   const int RL = q.K <= 5120 ? 4 : (q.K <= 10240 ? 2 : 1);
   if (q.had_block == 0 && q.K == 4096) {
-    if (q.asym) return write_codes ? launch_ring_split<4, true, true>(q) : cudaErrorInvalidValue;
-    return write_codes ? launch_ring_split<4, true, false>(q) : launch_ring_split<4, false, false>(q);
+    if (q.asym) {
+      if (q.sa != nullptr || !write_codes) return cudaErrorInvalidValue;
+      return launch_ring_split<4, true, true, false>(q);
+    }
+    if (q.sa != nullptr) {
+      return write_codes ? launch_ring_split<4, true, false, true>(q) : launch_ring_split<4, false, false, true>(q);
+    }
+    return write_codes ? launch_ring_split<4, true, false, false>(q) : launch_ring_split<4, false, false, false>(q);
   }
   if (q.had_block) {
     return write_codes ? launch_ring_hw<true, true>(q, V, RL) : launch_ring_hw<true, false>(q, V, RL);

@@ -92,14 +92,19 @@ def test_quantizer_hadamard_bit_exact(K, B):
 
 
 def test_quantizer_per_channel_sa_long_rows():
-    # K >= 4096 with a per-channel s^a vector takes the register-resident kernel, not the ring
+    # a per-channel s^a vector: the ring's split kernel at K = 4096 without Hadamard, the
+    # register-resident kernel otherwise
     rng = np.random.default_rng(17)
     for K in (4096, 11008):
         x = rand_x(rng, 9, K)
         b = (0.5 * rng.standard_normal(K)).astype(np.float32)
         sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
         check_quant(x, 0.9, 1.0, sa, b)
+        check_quant(x, 0.9, 1.0, sa, None)
         check_quant(x, 0.9, 1.0, sa, b, 128)
+    x = rand_x(rng, 1030, 4096)                  # many stages per CTA, ragged last stage
+    sa = (1.0 + 0.1 * rng.standard_normal(4096)).astype(np.float32)
+    check_quant(x, 0.9, 1.0, sa, (0.5 * rng.standard_normal(4096)).astype(np.float32))
 
 
 def test_quantizer_strided_input():
