@@ -322,6 +322,7 @@ def run_gpu(args):
     fused = run_fused(args, bq, torch, plan, acts, layers, T)
     asym = run_asym(args, bq, torch, plan, acts, layers, T)
     kv = run_kv(args, bq, torch, T, peaks["hbm_gbs"])
+    qcold = run_quant_cold(args, bq, torch, plan, acts, T, peaks["hbm_gbs"])
 
     # ---- end-to-end: HOST buffers through baseq_linear_host (H2D of X and D2H of Y timed)
     e2e = run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank)
@@ -333,7 +334,7 @@ def run_gpu(args):
             "data": "synthetic", "config": workload_config(config), "clocks": clocks,
             "e2e": e2e, "gpu_launches": nk * args.steps, "roofline": roofline,
             "roofline_quantizer": roofline_q, "kernels": per_layer, "fused_variant": fused,
-            "asym_variant": asym, "kv_quantizer": kv}
+            "asym_variant": asym, "kv_quantizer": kv, "quantizer_cold": qcold}
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(config, data, plan, layers, torch)
     if rank == 0:
@@ -428,6 +429,36 @@ def run_kv(args, bq, torch, T, hbm_gbs):
         gbs = by / (ms * 1e-3) / 1e9
         out.append({"shape": name, "T": T, "ms": ms, "GB_per_s": gbs, "frac_of_measured_hbm": gbs / hbm_gbs,
                     "bytes_per_element": 2.5, "buffers_rotated": nbuf})
+        del xs, outs
+    return out
+
+
+def run_quant_cold(args, bq, torch, plan, acts, T, hbm_gbs):
+    """the quantiser timed alone, cold -- back-to-back launches rotating over enough
+    (X, codes) buffer sets that the footprint exceeds 2 x L2 -- next to the in-step figure of
+    `roofline_quantizer` (which includes the gap after the preceding GEMM)."""
+    steps = max(10, min(args.steps, 40))
+    out = []
+    for act, _specs in plan:
+        a = acts[act]
+        K = a["K"]
+        by = 2.5 * T * K
+        nbuf = int(280e6 // by) + 2
+        xs = [a["x"]] + [a["x"].clone() for _ in range(nbuf - 1)]
+        outs = [(torch.empty_like(a["codes"]), torch.empty_like(a["scales"])) for _ in range(nbuf)]
+        for i in range(nbuf):
+            bq.quantize_act(xs[i], a["params"], *outs[i])
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(steps):
+            bq.quantize_act(xs[k % nbuf], a["params"], *outs[k % nbuf])
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        gbs = by / (ms * 1e-3) / 1e9
+        out.append({"name": act, "T": T, "K": K, "ms": ms, "GB_per_s": gbs,
+                    "frac_of_measured_hbm": gbs / hbm_gbs, "buffers_rotated": nbuf})
         del xs, outs
     return out
 
