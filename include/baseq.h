@@ -122,7 +122,8 @@ BASEQ_API baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scal
  *   s_t = max((alpha * (mx - mn)) / 15, 1e-12);  z_t = alpha * mn
  *   q_k = clamp(rne((u_k - z_t) * (1 / s_t)), 0, 15)            UNSIGNED codes, same nibble packing
  *   zeros  [T] fp32 lattice lower bounds z_t
- * The GEMM multiplies the unsigned codes by the signed weights (tcgen05 kind::i8, U8 x S8) and the
+ * The GEMM re-centres the unsigned codes to q - 8 on chip (tcgen05 kind::i8, S8 x S8, accumulating
+ * acc - 8 wsum; acc_dump still returns acc = sum_k q qw, the oracle's accumulator) and the
  * epilogue adds the lower-bound term:  Y = bf16_rne( fma(s_t s_w, acc, fma(z_t s_w, wsum[n], fb[n])) )
  * with wsum[n] = sum_k qw[n,k] from the packed blob (fp64 expression, one rounding to bf16).
  * p->sa must be NULL (scalar gamma only), else BASEQ_ERR_UNSUPPORTED; there is no fused variant. */
