@@ -64,7 +64,7 @@ BASEQ_API int baseq_version(void);
 /* The per-quantizer parameters of Eq. 15 / BlockParams.
  *   u_k = g_k * h_k - b_k,  h = block-Hadamard(x) or x,  g_k = sa ? sa[k] : gamma    (C-1, C-2)
  *   s_t = max((alpha * max_k |u_k|) / 7, 1e-12)                                       (C-7, C-8, C-10)
- *   q_k = clamp(rne(u_k * (1 / s_t)), -8, 7)                                          (C-5, C-6)
+ *   q_k = clamp(rne(u_k * (1 / s_t)), -8, 7)     product exact, one rounding     (C-5, C-6, C-17)
  * every line one correctly rounded fp32 operation. */
 typedef struct {
   float alpha;      /* clip ratio, 2^-16 <= alpha <= 1, else BASEQ_ERR_PARAM     */

@@ -156,15 +156,17 @@ int oracle_quantize_act(const uint16_t* x_bf16, int64_t ldx, int T, int K, float
     st = std::fmax(st, 1e-12f);
     // Q5: one reciprocal per row.
     float inv = 1.0f / st;
-    // Q6: r = u * inv; q = clamp(rint(r), -8, 7)   (Eq. 4: clip o round).
+    // Q6: q = clamp(rint(u * inv), -8, 7) with the product exact   (Eq. 4: clip o round).
     // Q7: pack two's-complement nibbles, low nibble = even k.
     for (int k = 0; k < K; k += 2) {
       int q2[2];
       for (int j = 0; j < 2; ++j) {
-        float r = u[k + j] * inv;
-        float rr = std::nearbyintf(r);       // default rounding mode: ties to even
-        if (rr < -8.0f) rr = -8.0f;
-        if (rr > 7.0f) rr = 7.0f;
+        // the product of two floats is exact in double (48 significant bits): ONE rounding, of
+        // the exact u * inv to an integer (Eq. 4 P:74 rounds the quotient once; reading C-17)
+        double r = static_cast<double>(u[k + j]) * static_cast<double>(inv);
+        double rr = std::nearbyint(r);       // default rounding mode: ties to even
+        if (rr < -8.0) rr = -8.0;
+        if (rr > 7.0) rr = 7.0;
         q2[j] = static_cast<int>(rr);
       }
       codes[static_cast<int64_t>(t) * (K / 2) + k / 2] =
@@ -263,7 +265,8 @@ int oracle_epilogue(const int32_t* acc, const float* scales, const float* w_scal
 // symmetric quantizer (Q0-Q2), then, each line one correctly rounded fp32 operation:
 //   A1  mn = min_k u_k, mx = max_k u_k
 //   A2  s_t = fmaxf((alpha * (mx - mn)) / 15, 1e-12);  z_t = alpha * mn;  inv = 1 / s_t
-//   A3  q_k = clamp(rint((u_k - z_t) * inv), 0, 15)          (unsigned code)
+//   A3  q_k = clamp(rint((u_k - z_t) * inv), 0, 15)          (unsigned code; the subtraction is one
+//       fp32 operation, the product is exact, rint rounds once)
 //   A4  byte j = q_2j | (q_2j+1 << 4)
 // Parity status: pinned (lattice row 0..15 -> z = 0, s = 1, codes = the integers;
 // constant row; reconstruction within s/2 for alpha = 1; reduces to an independent numpy
@@ -305,10 +308,10 @@ int oracle_quantize_act_asym(const uint16_t* x_bf16, int64_t ldx, int T, int K, 
       unsigned q2[2];
       for (int j = 0; j < 2; ++j) {
         float v = u[k + j] - z;
-        float r = v * inv;
-        float rr = std::nearbyintf(r);
-        if (rr < 0.0f) rr = 0.0f;
-        if (rr > 15.0f) rr = 15.0f;
+        double r = static_cast<double>(v) * static_cast<double>(inv);   // exact; one rounding (C-17)
+        double rr = std::nearbyint(r);
+        if (rr < 0.0) rr = 0.0;
+        if (rr > 15.0) rr = 15.0;
         q2[j] = static_cast<unsigned>(rr);
       }
       codes[static_cast<int64_t>(t) * (K / 2) + k / 2] = static_cast<uint8_t>(q2[0] | (q2[1] << 4));

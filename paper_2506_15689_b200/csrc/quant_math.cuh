@@ -98,12 +98,13 @@ __device__ __forceinline__ float step_size(float alpha, float absmax) {
 }
 __device__ __forceinline__ float reciprocal(float st) { return __fdiv_rn(1.0f, st); }
 
-// Q6: bits whose low nibble is the two's-complement code clamp(rne(u * inv), -8, 7)
-// (magic add: 1.5 * 2^23 + r has ulp 1, so the fp32 add performs the round-half-to-even).
+// Q6: bits whose low nibble is the two's-complement code clamp(rne(u * inv), -8, 7), the product
+// exact (reading C-17): fma(u, inv, 1.5 * 2^23) has ulp 1 in [2^23, 2^24), so its single rounding IS
+// the round-half-to-even of the exact product; the clamp acts on the biased value.
 __device__ __forceinline__ uint32_t code_bits(float u, float inv) {
-  float r = __fmul_rn(u, inv);
-  r = fminf(fmaxf(r, -8.0f), 7.0f);
-  return __float_as_uint(__fadd_rn(r, 12582912.0f));
+  float t = __fmaf_rn(u, inv, 12582912.0f);
+  t = fminf(fmaxf(t, 12582904.0f), 12582919.0f);           // magic - 8, magic + 7
+  return __float_as_uint(t);
 }
 
 // Q7: 8 codes -> one 32-bit word of nibbles (channel j in nibble j)
@@ -119,12 +120,12 @@ __device__ __forceinline__ uint32_t pack_nibbles(const uint32_t (&t)[8]) {
 
 
 // Q6 + Q7 for 8 channels at once.  |u * inv| <= 7 / alpha (1 + 2^-22) <= 7 * 2^16 < 2^22 because
-// |u| <= the row's absmax and the API requires alpha >= 2^-16, so the magic add is exact (RNE), the
-// integer subtract recovers the signed integer rne(r), and cvt.pack.sat.s4.s32 clamps it to
-// [-8, 7] and packs two codes per instruction:  d = (c << 8) | (sat(a) << 4) | (sat(b) & 15).
+// |u| <= the row's absmax and the API requires alpha >= 2^-16, so fma(u, inv, 1.5 * 2^23) stays in
+// [2^23, 2^24) and rounds the exact product to the nearest integer, ties to even; the integer
+// subtract recovers the signed integer, and cvt.pack.sat.s4.s32 clamps it to [-8, 7] and packs two
+// codes per instruction:  d = (c << 8) | (sat(a) << 4) | (sat(b) & 15).
 __device__ __forceinline__ int32_t code_int(float u, float inv) {
-  const float r = __fmul_rn(u, inv);
-  return static_cast<int32_t>(__float_as_uint(__fadd_rn(r, 12582912.0f))) - 0x4B400000;
+  return static_cast<int32_t>(__float_as_uint(__fmaf_rn(u, inv, 12582912.0f))) - 0x4B400000;
 }
 __device__ __forceinline__ uint32_t pack2_sat(int32_t hi, int32_t lo, uint32_t prev) {
   uint32_t d;
@@ -146,12 +147,12 @@ __device__ __forceinline__ float step_size_asym(float alpha, float mn, float mx)
   return fmaxf(__fdiv_rn(__fmul_rn(alpha, __fsub_rn(mx, mn)), 15.0f), 1e-12f);
 }
 __device__ __forceinline__ float lower_bound_asym(float alpha, float mn) { return __fmul_rn(alpha, mn); }
-// The lower clamp is done in floating point (rne is monotone and rne(0) = 0, so clamping before
-// rounding is the same thing; it also keeps the magic add away from its wrap-around), the upper
+// The lower clamp is done in floating point on the biased value (a negative product must not reach
+// the integer subtract as a value below 2^23, where the ulp is no longer 1), the upper
 // one by the saturating pack:  d = (c << 8) | (sat_u4(a) << 4) | sat_u4(b).
 __device__ __forceinline__ int32_t code_int_asym(float u, float z, float inv) {
-  const float r = fmaxf(__fmul_rn(__fsub_rn(u, z), inv), 0.0f);
-  return static_cast<int32_t>(__float_as_uint(__fadd_rn(r, 12582912.0f))) - 0x4B400000;
+  const float t = fmaxf(__fmaf_rn(__fsub_rn(u, z), inv, 12582912.0f), 12582912.0f);
+  return static_cast<int32_t>(__float_as_uint(t)) - 0x4B400000;
 }
 __device__ __forceinline__ uint32_t pack2_sat_u(int32_t hi, int32_t lo, uint32_t prev) {
   uint32_t d;

@@ -142,7 +142,7 @@ def _rtn_independent(xf, alpha):
     m = np.max(np.abs(xf), axis=1).astype(np.float32)
     s = np.maximum((np.float32(alpha) * m) / np.float32(7.0), np.float32(1e-12)).astype(np.float32)
     inv = (np.float32(1.0) / s).astype(np.float32)
-    r = (xf * inv[:, None]).astype(np.float32)
+    r = xf.astype(np.float64) * inv[:, None].astype(np.float64)      # exact product, one rounding (C-17)
     q = np.clip(np.rint(r), -8, 7).astype(np.int32)
     return q, s
 
@@ -521,7 +521,7 @@ def test_asym_matches_independent_restatement_and_reconstructs():
         st = np.maximum((np.float32(alpha) * (mx - mn)) / np.float32(15.0), np.float32(1e-12)).astype(np.float32)
         zz = (np.float32(alpha) * mn).astype(np.float32)
         inv = (np.float32(1.0) / st).astype(np.float32)
-        q = np.clip(np.rint(((u - zz[:, None]).astype(np.float32) * inv[:, None]).astype(np.float32)), 0, 15)
+        q = np.clip(np.rint((u - zz[:, None]).astype(np.float32).astype(np.float64) * inv[:, None].astype(np.float64)), 0, 15)
         assert np.array_equal(s.view(np.uint32), st.view(np.uint32))
         assert np.array_equal(z.view(np.uint32), zz.view(np.uint32))
         assert np.array_equal(ucodes(c), q.astype(np.int64))
@@ -590,3 +590,37 @@ def test_kv_lattice_heads_exact_and_reconstruct():
     assert np.all(np.abs(rec - xf) <= 0.5 * np.repeat(s, D, axis=1) * (1 + 2.0 ** -18))
     # and the steps really are per head: they follow the heads' spreads
     assert np.all(s[:, 0] < s[:, 1]) and np.all(s[:, 1] < s[:, 2]) and np.all(s[:, 2] < s[:, 3])
+
+
+def test_rounding_is_of_the_exact_product():
+    # C-17: q = rne(u * inv) rounds the EXACT product once.  Steer inv with alpha until the exact
+    # u * inv lies strictly on one side of k + 1/2 while its fp32-rounded value is the tie itself
+    # (a separately rounded product would then go to the even neighbour): the code must follow the
+    # exact product.
+    f32 = np.float32
+    m = f32(8.0)
+    found = {"below": 0, "above": 0}
+    separating = 0        # cases where rounding the fp32 product (ties to even) gives another code
+    # bf16-representable u with full 8-bit significands, |u| < m; odd and even k
+    for u, k in ((f32(191 / 128), 1), (f32(147 / 128), 2), (f32(221 / 128), 3), (f32(1.5), 4),
+                 (f32(253 / 128), 5), (f32(163 / 128), 6)):
+        a0 = f32(7.0 * (float(u) / (k + 0.5)) / float(m))
+        alpha = a0
+        for _ in range(64):
+            alpha = np.nextafter(alpha, f32(0.0))
+        for _ in range(129):
+            st = f32(f32(alpha * m) / f32(7.0))
+            inv = f32(f32(1.0) / st)
+            exact = float(u) * float(inv)           # exact in double: 8 x 24 significant bits
+            if f32(exact) == f32(k + 0.5) and exact != k + 0.5 and 2.0 ** -16 <= alpha <= 1.0:
+                row = np.zeros((1, 128), dtype=f32)
+                row[0, 0], row[0, 1] = m, u
+                c, s = oracle.quantize_act(bf16(row), float(alpha))
+                assert s[0] == st
+                side = "above" if exact > k + 0.5 else "below"
+                assert codes_to_int(c)[0, 1] == (k + 1 if side == "above" else k)
+                found[side] += 1
+                separating += (side == "above") == (k % 2 == 0)
+            alpha = np.nextafter(alpha, f32(2.0))
+    assert found["below"] > 0 and found["above"] > 0     # the search exercised both sides
+    assert separating > 0
