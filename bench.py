@@ -323,6 +323,7 @@ def run_gpu(args):
     asym = run_asym(args, bq, torch, plan, acts, layers, T)
     kv = run_kv(args, bq, torch, T, peaks["hbm_gbs"])
     qcold = run_quant_cold(args, bq, torch, plan, acts, T, peaks["hbm_gbs"])
+    decode = run_decode(args, bq, torch, plan, data, acts, layers, peaks["hbm_gbs"])
 
     # ---- end-to-end: HOST buffers through baseq_linear_host (H2D of X and D2H of Y timed)
     e2e = run_e2e(args, bq, torch, plan, data, acts, layers, T, ws, local_rank)
@@ -334,7 +335,8 @@ def run_gpu(args):
             "data": "synthetic", "config": workload_config(config), "clocks": clocks,
             "e2e": e2e, "gpu_launches": nk * args.steps, "roofline": roofline,
             "roofline_quantizer": roofline_q, "kernels": per_layer, "fused_variant": fused,
-            "asym_variant": asym, "kv_quantizer": kv, "quantizer_cold": qcold}
+            "asym_variant": asym, "kv_quantizer": kv, "quantizer_cold": qcold,
+            "decode_shapes": decode}
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(config, data, plan, layers, torch)
     if rank == 0:
@@ -460,6 +462,72 @@ def run_quant_cold(args, bq, torch, plan, acts, T, hbm_gbs):
         out.append({"name": act, "T": T, "K": K, "ms": ms, "GB_per_s": gbs,
                     "frac_of_measured_hbm": gbs / hbm_gbs, "buffers_rotated": nbuf})
         del xs, outs
+    return out
+
+
+def run_decode(args, bq, torch, plan, data, acts, layers, hbm_gbs):
+    """the same layers at decode token counts.  T <= 64 takes the W-streaming
+    kernel (w4a4_decode.cu) behind baseq_w4a4_gemm; T = 65 is the tcgen05 kernel on one tile row,
+    listed for comparison.  Cold weights: the steps rotate over enough packed copies of the layer
+    set that the footprint exceeds 2 x L2.  HBM-bound: algorithmic bytes per GEMM =
+    N K / 2 (packed W) + T K / 2 (codes) + 2 T N (Y)."""
+    steps = max(10, min(args.steps, 50))
+    if min(a["x"].shape[0] for a in acts.values()) < 65:
+        return []          # c1: the whole workload is already a decode shape
+
+    def dev(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    w_bytes = sum(sp.N * sp.K / 2 for _a, specs in plan for sp in specs)
+    ncopy = int(280e6 // w_bytes) + 2
+    copies = [{sp.name: layers[sp.name]["pw"] for _a, specs in plan for sp in specs}]
+    for _ in range(ncopy - 1):
+        c = {}
+        for act, specs in plan:
+            for sp in specs:
+                W = data["weights"][sp.name]
+                c[sp.name] = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(data["acts"][act]["b"]),
+                                             None if W["layer_bias"] is None else dev(W["layer_bias"]))
+        copies.append(c)
+    torch.cuda.synchronize()
+    out = []
+    for Td in (1, 8, 16, 32, 64, 65):
+        bufs = {}
+        for act, specs in plan:
+            a = acts[act]
+            bufs[act] = (a["x"][:Td], torch.empty((Td, a["K"] // 2), dtype=torch.uint8, device="cuda"),
+                         torch.empty((Td,), dtype=torch.float32, device="cuda"))
+            for sp in specs:
+                bufs[sp.name] = torch.empty((Td, sp.N), dtype=torch.bfloat16, device="cuda")
+
+        def step(k, with_quant):
+            pws = copies[k % ncopy]
+            for act, specs in plan:
+                x, codes, scales = bufs[act]
+                if with_quant:
+                    bq.quantize_act(x, acts[act]["params"], codes, scales)
+                for sp in specs:
+                    bq.w4a4_gemm(codes, scales, pws[sp.name], bufs[sp.name])
+
+        res = {}
+        for with_quant in (True, False):
+            for k in range(ncopy):
+                step(k, with_quant)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for k in range(steps):
+                step(k, with_quant)
+            e1.record()
+            torch.cuda.synchronize()
+            res[with_quant] = e0.elapsed_time(e1) / steps
+        by = sum(sp.N * sp.K / 2 + Td * sp.K / 2 + 2.0 * Td * sp.N for _a, specs in plan for sp in specs)
+        gbs = by / (res[False] * 1e-3) / 1e9
+        out.append({"T": Td, "kernel": "w4a4_decode_kernel" if Td <= 64 else "w4a4_gemm_kernel (tcgen05)",
+                    "step_ms": res[True], "tokens_per_s": Td / (res[True] * 1e-3),
+                    "gemms_ms": res[False], "gemm_GB_per_s": gbs, "frac_of_measured_hbm": gbs / hbm_gbs,
+                    "weight_copies_rotated": ncopy})
+    del copies
     return out
 
 

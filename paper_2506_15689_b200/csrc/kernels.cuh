@@ -118,5 +118,9 @@ struct GemmLaunch {
 };
 // Returns cudaSuccess, or an error (cudaErrorNotSupported when the tensor map cannot be built).
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g);
+// Decode shapes (NEXT-4, w4a4_decode.cu): the same contract and the same bits for T <= kDecodeMaxT,
+// bound by streaming the packed weights once; launch_w4a4_gemm routes the unfused calls there.
+constexpr int kDecodeMaxT = 64;
+cudaError_t launch_w4a4_decode(const GemmLaunch& g);
 
 }  // namespace baseq

@@ -34,6 +34,7 @@
 // (|256 * acc| <= 256 * 64 * K < 2^31 for K <= 131072); acc = raw >> 8 is exact.
 #include <cuda.h>
 
+#include "epilogue_math.cuh"
 #include "kernels.cuh"
 #include "ptx.cuh"
 #include "quant_math.cuh"
@@ -149,23 +150,12 @@ __device__ __forceinline__ void advance(int& stage, uint32_t& phase, int n) {
 //   |y - y*| <= 2^-24 (|t s_w| + |y|) (1 + eps)  <  E := 2^-23 (|RN(t s_w)| + |y|)
 // If bf16(y - E) == bf16(y + E) every real number in the bracket -- including the fp64 value --
 // rounds to that bf16.
-__device__ __forceinline__ uint32_t bf16_from_double_rne(double v) {
-  // round-to-odd to fp32 (keeps a sticky bit), then RNE to bf16: a single rounding overall
-  float f = __double2float_rz(v);
-  uint32_t u = __float_as_uint(f);
-  if (static_cast<double>(f) != v) u |= 1u;
-  const uint32_t r = u + 0x7FFFu + ((u >> 16) & 1u);
-  return r >> 16;
-}
-
 // One output.  Fast path: t = RN(s_t * accf), p = RN(t * s_w), y = RN(t * s_w + fb) and the
 // bracket [y - E, y + E] with E = 2^-23 (|p| + |y|) >= 2 |y - y*| (see above); when both ends round
 // to the same bf16 (all but ~2.4e-4 of the elements, whatever the cancellation between p and fb)
 // that is the result, otherwise the fp64 expression itself is evaluated.
 __device__ __noinline__ uint32_t dequant_f64(int32_t acc, float st, float sw, float fb) {
-  const double pd = __dmul_rn(static_cast<double>(st), static_cast<double>(sw));
-  const double yd = __fma_rn(pd, static_cast<double>(acc), static_cast<double>(fb));
-  return bf16_from_double_rne(yd);
+  return epi::dequant_f64(acc, st, sw, fb);
 }
 // `raw` is the TMEM accumulator 256 * acc (|acc| < 2^22, so raw has at most 22 significant bits
 // and converts to fp32 exactly) and st256 = s_t * 2^-8 (exact): st256 * float(raw) is the same
@@ -204,12 +194,7 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float a1, float a0) {
 // exactly as acc' + 8 wsum.
 __device__ __noinline__ uint32_t dequant_f64_asym(int32_t acc_c, float st, float zt, float sw,
                                                   float fb, float ws) {
-  const int32_t acc = acc_c + 8 * static_cast<int32_t>(ws);
-  const double swd = static_cast<double>(sw);
-  const double c = __fma_rn(__dmul_rn(static_cast<double>(zt), swd), static_cast<double>(ws),
-                            static_cast<double>(fb));
-  const double yd = __fma_rn(__dmul_rn(static_cast<double>(st), swd), static_cast<double>(acc), c);
-  return bf16_from_double_rne(yd);
+  return epi::dequant_f64_asym(acc_c, st, zt, sw, fb, ws);
 }
 __device__ __forceinline__ void dequant_bracket_asym(int32_t raw, float st256, float midf, float sw,
                                                      float fb, float ws, float& lo, float& hi) {
@@ -813,6 +798,7 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, cons
 
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   const bool fused = g.x != nullptr;
+  if (!fused && g.T <= kDecodeMaxT) return launch_w4a4_decode(g);   // decode shapes: W-streaming kernel
   if (fused && g.had_block > 128) return cudaErrorNotSupported;   // 16 lanes hold 128 channels
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);

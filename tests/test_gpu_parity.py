@@ -492,3 +492,85 @@ def test_kv_rejects_other_head_dims():
     x = torch.zeros((4, 96 * 2), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(bq.BaseqError):
         bq.quantize_kv(x, 2, 96)
+
+
+# ------------------------------------------------------------------------------- NEXT-4: decode shapes
+# T <= 64 takes the W-streaming decode kernel (w4a4_decode.cu) behind the same baseq_w4a4_gemm /
+# baseq_w4a4_gemm_asym calls; same contract, same bits.
+@pytest.mark.parametrize("T", [1, 7, 8, 9, 16, 17, 32, 33, 63, 64])
+def test_decode_token_counts(T):
+    # every token-tile instantiation (8 / 16 / 32 / 64), ragged token tails, N % 16 == 8,
+    # K = 11 k-blocks (8 warps: three take two k-blocks, five take one)
+    rng = np.random.default_rng(100 + T)
+    K, N = 1408, 200
+    x = rand_x(rng, T, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    W = _rand_w(rng, N, K)
+    run_linear(x, W, 0.9, 1.05, b)
+    run_asym(x, W, 0.9, 1.05, b)
+
+
+@pytest.mark.parametrize("T,K,N", [(1, 128, 8), (5, 256, 96), (64, 4096, 112), (16, 11008, 208),
+                                   (24, 28672, 64), (40, 4224, 1000)])
+def test_decode_k_and_n_edges(T, K, N):
+    # one k-block (seven idle warps), several rounds of the in-flight window (K = 28672: 224
+    # k-blocks), row groups at the end of / across 96-row weight boxes, N below one group
+    rng = np.random.default_rng(T + 3 * K + 11 * N)
+    x = rand_x(rng, T, K, spread=1.0)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    W = _rand_w(rng, N, K)
+    run_linear(x, W, 0.9, 1.0, b)
+    run_asym(x, W, 1.0, 1.0, b)
+
+
+def test_decode_extreme_codes():
+    # largest raw accumulators: qa = -8, qw = -8 -> acc = 64 K; qa = 7, qw = -8 -> -56 K (closed forms)
+    T, K, N = 48, 28672, 64
+    scales = torch.full((T,), 0.25, dtype=torch.float32, device="cuda")
+    wn = np.full((N, K // 2), 0x88, dtype=np.uint8)
+    pw = bq.pack_weights(dev(wn), dev(np.full((N,), 0.5, dtype=np.float32)))
+    for byte, per_k in ((0x88, 64), (0x77, -56)):
+        codes = torch.full((T, K // 2), byte, dtype=torch.uint8, device="cuda")
+        acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
+        y = bq.w4a4_gemm(codes, scales, pw, acc_dump=acc)
+        torch.cuda.synchronize()
+        assert torch.all(acc == per_k * K)
+        assert torch.all(y.float() == float(torch.tensor(per_k * K * 0.125).bfloat16()))
+
+
+def test_decode_matches_prefill_kernel_on_shared_rows():
+    # the same codes through both kernels: rows 0..T-1 of a 130-token call (tcgen05 GEMM) and a
+    # T-token call (decode kernel) must agree bit for bit, Llama-2-7B q/k/v/o shape, full N
+    L = make_layer("c2", "qkvo", T=130)
+    sp = L["spec"]
+    pw = bq.pack_weights(dev(L["w_nibbles"]), dev(L["w_scale"]), dev(L["b"]),
+                         None if L["layer_bias"] is None else dev(L["layer_bias"]))
+    params = bq.ActParams(sp.alpha, sp.gamma, None, dev(L["b"]), sp.had_block)
+    codes, scales = bq.quantize_act(bf16_dev(L["x"]), params)
+    y_big = bq.w4a4_gemm(codes, scales, pw)
+    for T in (1, 8, 20, 64):
+        acc = torch.empty((T, sp.N), dtype=torch.int32, device="cuda")
+        y = bq.w4a4_gemm(codes[:T].contiguous(), scales[:T].contiguous(), pw, acc_dump=acc)
+        torch.cuda.synchronize()
+        assert torch.equal(y.view(torch.int16), y_big[:T].view(torch.int16)), T
+    # and against the oracle on the first two tokens
+    fb = oracle.fused_bias(L["w_nibbles"], L["w_scale"], L["b"], L["layer_bias"])
+    ref = oracle.linear(np.ascontiguousarray(L["x"][:2]), L["w_nibbles"], L["w_scale"], fb,
+                        sp.alpha, sp.gamma, None, L["b"], sp.had_block)
+    assert np.array_equal(bits_host(y_big[:2]), ref["y"])
+
+
+def test_decode_strided_output():
+    # ldy > N: the decode kernel writes only the N columns of each row
+    rng = np.random.default_rng(77)
+    T, K, N = 12, 512, 136
+    x = rand_x(rng, T, K)
+    W = _rand_w(rng, N, K)
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None, dev(W["layer_bias"]))
+    codes, scales = bq.quantize_act(bf16_dev(x), bq.ActParams(0.9))
+    y_ref = bq.w4a4_gemm(codes, scales, pw)
+    buf = torch.full((T, 160), -1.0, dtype=torch.bfloat16, device="cuda")
+    bq.w4a4_gemm(codes, scales, pw, y=buf[:, :N])
+    torch.cuda.synchronize()
+    assert torch.equal(buf[:, :N].contiguous().view(torch.int16), y_ref.view(torch.int16))
+    assert torch.all(buf[:, N:] == -1.0)
