@@ -110,7 +110,14 @@ BASEQ_API baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int
  *   codes, scales  as produced by baseq_quantize_act
  *   packed_w       blob from baseq_pack_weights for the same (N, K)
  *   y_bf16         [T, ldy] bf16 row-major
- *   acc_dump       optional [T, N] int32 copy of the accumulators (parity runs only), or NULL */
+ *   acc_dump       optional [T, N] int32 copy of the accumulators (parity runs only), or NULL
+ * Decode shapes: for T <= 64 this call and baseq_w4a4_gemm_asym run a
+ * weight-streaming kernel (one pass over the packed weights, warp-level s8 MMA on nibbles
+ * expanded in registers) instead of the tcgen05 tile kernel; same contract, same bits, same
+ * arguments -- the choice is not visible to the caller.  Both kernels are enqueued with the
+ * programmatic-dependent-launch attribute and read `codes` / `scales` only after the preceding
+ * kernel of `stream` has completed; inside a CUDA graph consecutive calls overlap their weight
+ * streams. */
 BASEQ_API baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const void* packed_w,
                                int T, int N, int K, void* y_bf16, int64_t ldy, int32_t* acc_dump,
                                void* stream);

@@ -3,11 +3,14 @@
 // work is streaming the packed weights once (N K / 2 bytes) and the 128 x 192 tcgen05 tile would
 // be 1-50 % full.  HBM-bound: algorithmic bytes = N K / 2 (W) + T K / 2 (codes) + 2 T N (Y).
 //
-//   CTA            one group of 16 output channels (16 rows x 64 bytes = 1 KB contiguous per k-block
-//                  of the weight blob), all of K, all T tokens; grid = ceil(N / 16)
-//   8 warps        k-blocks w, w + 8, ... each; kDepth k-blocks of W (2 x LDG.128 per lane and
-//                  k-block, streaming, issued BEFORE griddepcontrol.wait: the weights do not depend
-//                  on the preceding quantiser) are in flight per warp
+//   CTA            MT groups of 16 output channels (MT = 2 for T > 16 and N >= 64 SMs, else 1; a group is 16 rows x
+//                  64 bytes = 1 KB contiguous per k-block of the weight blob), all of K, all T
+//                  tokens; grid = ceil(N / (16 MT))
+//   8 warps        k-blocks w, w + 8, ... each, through a rolling window of kDepth register slots
+//                  (2 MT x LDG.128 per lane and k-block, streaming; the first window is issued
+//                  BEFORE griddepcontrol.wait: the weights do not depend on the preceding
+//                  quantiser, and griddepcontrol.launch_dependents right after it lets a following
+//                  decode GEMM stream its weights while this one drains)
 //   MMA            mma.sync.m16n8k32 s8 x s8 -> s32 with M = output channels, N = 8 tokens: at
 //                  T <= 64 the contraction is 0.4-3 % of the tensor peak, the legacy warp-level MMA
 //                  is ample and needs no shared-memory operand staging
@@ -17,8 +20,9 @@
 //                  its partner (a permutation of k inside the dot product); raw = 256 acc exactly.
 //                  Asymmetric codes (NEXT-1, unsigned) are re-centred to q - 8 by flipping the top
 //                  bit, as in the tcgen05 kernel.
-//   epilogue       partial sums of the 8 warps meet in shared memory; every output is evaluated
-//                  with the fp64 expression of the contract itself (<= 1024 outputs per CTA).
+//   epilogue       the 8 partial sums meet in shared memory (integer atomics: order-free); every
+//                  output is evaluated with the fp64 expression of the contract itself
+//                  (<= 2048 outputs per CTA), 32-64 contiguous bytes of a Y row per half-warp / warp.
 #include "epilogue_math.cuh"
 #include "kernels.cuh"
 #include "ptx.cuh"
@@ -26,10 +30,7 @@
 namespace baseq {
 namespace {
 
-constexpr int kWarps = 8;
-constexpr int kThreads = kWarps * 32;
 constexpr int kRows = 16;          // output channels per CTA (MMA M)
-constexpr int kDepth = 4;          // k-blocks of W in flight per warp
 
 struct DecodeParams {
   const uint8_t* tiles;
@@ -58,47 +59,78 @@ __device__ __forceinline__ uint32_t word(const uint4& v, int i) {
   return i == 0 ? v.x : i == 1 ? v.y : i == 2 ? v.z : v.w;
 }
 
-// NT = token tiles of 8 (T <= 8 NT)
-template <int NT, bool ASYM>
-__global__ void __launch_bounds__(kThreads) w4a4_decode_kernel(const DecodeParams p) {
-  __shared__ int32_t red[kWarps][NT * 4 * 32];
+// NT = token tiles of 8 (T <= 8 NT); MT = groups of 16 output channels per CTA (a warp multiplies
+// all of them with the same activation fragments); kWarps warps split K; kDepth k-blocks of W in
+// flight per warp.
+template <int NT, int MT, bool ASYM, int kWarps, int kDepth>
+__global__ void __launch_bounds__(kWarps * 32, NT == 1 ? 3 : (NT * MT <= 8 ? 2 : 1)) w4a4_decode_kernel(const DecodeParams p) {
+  constexpr int kThreads = kWarps * 32;
+  constexpr int kCh = kRows * MT;                       // output channels per CTA
+  constexpr int kOut = (NT * 8 * kCh + kThreads - 1) / kThreads;   // outputs per thread
+  static_assert(kThreads % kCh == 0, "epilogue mapping");
+  __shared__ int32_t red[MT * NT * 4 * 32];
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t4 = lane & 3;
-  const int n0 = blockIdx.x * kRows;
-  // weight rows g and g + 8 of this group, k-block 0 (boxes of kTileRows rows x 64 bytes)
+  const int n0 = blockIdx.x * kCh;
+  // weight rows g and g + 8 of the first group, k-block 0 (boxes of kTileRows rows x 64 bytes);
+  // group m is 16 rows = 1 KB further on in the same box
   const uint8_t* wrow = p.tiles +
       (static_cast<size_t>(n0 / kTileRows) * p.num_kb * kTileRows + (n0 % kTileRows) + g) * 64 + t4 * 16;
   const uint8_t* xrow = p.codes + static_cast<size_t>(g) * (p.K / 2) + t4 * 16;
 
-  int32_t acc[NT][4];
-#pragma unroll
-  for (int j = 0; j < NT; ++j)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) acc[j][c] = 0;
+  // epilogue: this thread's outputs are one channel (ch) x tokens tok0 + i * (kThreads / kCh); the
+  // per-channel operands come from the weight blob and are requested first
+  const int ch = threadIdx.x % kCh, tok0 = threadIdx.x / kCh;
+  const int n = n0 + ch;
+  const bool n_ok = n < p.N;
+  const float sw = n_ok ? p.sw[n] : 0.0f, fb = n_ok ? p.fb[n] : 0.0f;
+  const float ws = (ASYM && n_ok) ? p.wsum[n] : 0.0f;
+  for (int i = threadIdx.x; i < MT * NT * 4 * 32; i += kThreads) red[i] = 0;
 
-  bool waited = false;
-  for (int kb0 = warp; kb0 < p.num_kb; kb0 += kWarps * kDepth) {
-    uint4 wa[kDepth], wb[kDepth];
+  int32_t acc[MT][NT][4];
+#pragma unroll
+  for (int m = 0; m < MT; ++m)
+#pragma unroll
+    for (int j = 0; j < NT; ++j)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) acc[m][j][c] = 0;
+
+  // this warp's k-blocks: warp, warp + kWarps, ... (`count` of them), consumed through a rolling
+  // window of kDepth register slots: slot d is refilled with k-block it + kDepth as soon as
+  // k-block it has been multiplied, so kDepth loads stay in flight until the row group ends
+  const int count = (p.num_kb - warp + kWarps - 1) / kWarps;
+  uint4 wa[kDepth][MT], wb[kDepth][MT];
+  auto load_w = [&](int d, int it) {
+    const uint8_t* src = wrow + static_cast<size_t>(warp + it * kWarps) * (kTileRows * 64);
+#pragma unroll
+    for (int m = 0; m < MT; ++m) {
+      wa[d][m] = ptx::ldg_nc_stream(reinterpret_cast<const uint4*>(src + m * (kRows * 64)));
+      wb[d][m] = ptx::ldg_nc_stream(reinterpret_cast<const uint4*>(src + m * (kRows * 64) + 8 * 64));
+    }
+  };
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) {
+#pragma unroll
+    for (int m = 0; m < MT; ++m) {
+      wa[d][m] = make_uint4(0, 0, 0, 0);
+      wb[d][m] = make_uint4(0, 0, 0, 0);
+    }
+    if (d < count) load_w(d, d);
+  }
+  // The first window of W is in flight.  Let the next kernel of the stream start on the SMs this
+  // grid leaves free (a following decode GEMM streams ITS weights meanwhile; every kernel of this
+  // library writes only after its own griddepcontrol.wait), then wait for the preceding kernel:
+  // codes and scales are its output.
+  ptx::griddep_launch_dependents();
+  ptx::griddep_wait();
+
+  for (int base = 0; base < count; base += kDepth) {
 #pragma unroll
     for (int d = 0; d < kDepth; ++d) {
-      const int kb = kb0 + d * kWarps;
-      wa[d] = make_uint4(0, 0, 0, 0);
-      wb[d] = make_uint4(0, 0, 0, 0);
-      if (kb < p.num_kb) {
-        const uint8_t* src = wrow + static_cast<size_t>(kb) * (kTileRows * 64);
-        wa[d] = ptx::ldg_nc_stream(reinterpret_cast<const uint4*>(src));
-        wb[d] = ptx::ldg_nc_stream(reinterpret_cast<const uint4*>(src + 8 * 64));
-      }
-    }
-    if (!waited) {
-      ptx::griddep_wait();      // codes and scales are the preceding kernel's output
-      waited = true;
-    }
-#pragma unroll
-    for (int d = 0; d < kDepth; ++d) {
-      const int kb = kb0 + d * kWarps;
-      if (kb < p.num_kb) {
+      const int it = base + d;
+      if (it < count) {
+        const int kb = warp + it * kWarps;
         uint4 xa[NT];
 #pragma unroll
         for (int j = 0; j < NT; ++j) {
@@ -109,9 +141,13 @@ __global__ void __launch_bounds__(kThreads) w4a4_decode_kernel(const DecodeParam
         }
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          const uint32_t a = word(wa[d], i), b = word(wb[d], i);
-          const uint32_t a0 = (a << 4) & 0xF0F0F0F0u, a2 = a & 0xF0F0F0F0u;
-          const uint32_t a1 = (b << 4) & 0xF0F0F0F0u, a3 = b & 0xF0F0F0F0u;
+          uint32_t a0[MT], a1[MT], a2[MT], a3[MT];
+#pragma unroll
+          for (int m = 0; m < MT; ++m) {
+            const uint32_t a = word(wa[d][m], i), b = word(wb[d][m], i);
+            a0[m] = (a << 4) & 0xF0F0F0F0u, a2[m] = a & 0xF0F0F0F0u;
+            a1[m] = (b << 4) & 0xF0F0F0F0u, a3[m] = b & 0xF0F0F0F0u;
+          }
 #pragma unroll
           for (int j = 0; j < NT; ++j) {
             const uint32_t x = word(xa[j], i);
@@ -120,50 +156,61 @@ __global__ void __launch_bounds__(kThreads) w4a4_decode_kernel(const DecodeParam
               b0 ^= 0x80808080u;        // 16 q -> 16 (q - 8) as int8
               b1 ^= 0x80808080u;
             }
-            mma_s8(acc[j], a0, a1, a2, a3, b0, b1);
+#pragma unroll
+            for (int m = 0; m < MT; ++m) mma_s8(acc[m][j], a0[m], a1[m], a2[m], a3[m], b0, b1);
           }
         }
+        if (it + kDepth < count) load_w(d, it + kDepth);
       }
     }
   }
-  if (!waited) ptx::griddep_wait();
 
+  // per-token epilogue operands, requested before the partial sums meet
+  float st[kOut], zt[kOut];
 #pragma unroll
-  for (int j = 0; j < NT; ++j)
+  for (int i = 0; i < kOut; ++i) {
+    const int tok = tok0 + i * (kThreads / kCh);
+    st[i] = tok < p.T ? p.scales[tok] : 0.0f;
+    zt[i] = (ASYM && tok < p.T) ? p.zeros[tok] : 0.0f;
+  }
+
+  // the kWarps partial sums meet in shared memory (integer adds: any order, same result)
+  __syncthreads();                                        // red is zero
 #pragma unroll
-    for (int c = 0; c < 4; ++c) red[warp][(j * 4 + c) * 32 + lane] = acc[j][c];
+  for (int m = 0; m < MT; ++m)
+#pragma unroll
+    for (int j = 0; j < NT; ++j)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) atomicAdd(&red[((m * NT + j) * 4 + c) * 32 + lane], acc[m][j][c]);
   __syncthreads();
 
-  // thread o -> (token, channel): 16 consecutive lanes write 32 contiguous bytes of one Y row
-  for (int o = threadIdx.x; o < NT * 8 * kRows; o += kThreads) {
-    const int tok = o >> 4, ch = o & 15;
-    const int n = n0 + ch;
-    if (tok >= p.T || n >= p.N) continue;
-    // accumulator fragment: c0, c1 = row g, tokens 2 t4 + {0, 1}; c2, c3 = row g + 8
-    const int j = tok >> 3, col = tok & 7;
-    const int idx = (j * 4 + (ch >> 3) * 2 + (col & 1)) * 32 + (ch & 7) * 4 + (col >> 1);
-    int32_t raw = 0;
+  // thread -> (token, channel): kCh consecutive threads write 2 kCh contiguous bytes of one Y row
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) raw += red[w][idx];
-    int32_t a = raw >> 8;                                  // raw = 256 acc exactly
-    const float st = p.scales[tok], sw = p.sw[n], fb = p.fb[n];
+  for (int i = 0; i < kOut; ++i) {
+    const int tok = tok0 + i * (kThreads / kCh);
+    if (tok >= NT * 8 || tok >= p.T || !n_ok) continue;
+    // accumulator fragment: c0, c1 = row g, tokens 2 t4 + {0, 1}; c2, c3 = row g + 8
+    const int j = tok >> 3, col = tok & 7, m = ch >> 4, r = ch & 15;
+    const int idx = ((m * NT + j) * 4 + (r >> 3) * 2 + (col & 1)) * 32 + (r & 7) * 4 + (col >> 1);
+    int32_t a = red[idx] >> 8;                             // raw = 256 acc exactly
     uint32_t out;
     if (ASYM) {
-      const float ws = p.wsum[n];
-      out = epi::dequant_f64_asym(a, st, p.zeros[tok], sw, fb, ws);
+      out = epi::dequant_f64_asym(a, st[i], zt[i], sw, fb, ws);
       a += 8 * static_cast<int32_t>(ws);                   // the accumulator over the unsigned codes
     } else {
-      out = epi::dequant_f64(a, st, sw, fb);
+      out = epi::dequant_f64(a, st[i], sw, fb);
     }
     p.y[static_cast<size_t>(tok) * p.ldy + n] = static_cast<uint16_t>(out);
     if (p.acc_dump != nullptr) p.acc_dump[static_cast<size_t>(tok) * p.N + n] = a;
   }
 }
 
-template <int NT, bool ASYM>
+// kDepth x MT = 4: the same bytes of W in flight per warp either way.
+template <int NT, int MT, bool ASYM>
 cudaError_t launch_nt(const DecodeParams& p, cudaStream_t stream) {
+  constexpr int kWarps = 8, kThreads = kWarps * 32, kDepth = 4 / MT;
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(static_cast<unsigned>((p.N + kRows - 1) / kRows), 1, 1);
+  cfg.gridDim = dim3(static_cast<unsigned>((p.N + kRows * MT - 1) / (kRows * MT)), 1, 1);
   cfg.blockDim = dim3(kThreads, 1, 1);
   cfg.dynamicSmemBytes = 0;
   cfg.stream = stream;
@@ -172,15 +219,20 @@ cudaError_t launch_nt(const DecodeParams& p, cudaStream_t stream) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, w4a4_decode_kernel<NT, ASYM>, p);
+  return cudaLaunchKernelEx(&cfg, w4a4_decode_kernel<NT, MT, ASYM, kWarps, kDepth>, p);
 }
 
+// T <= 16: one 16-channel group per CTA.  T > 16: two groups per CTA share the activation
+// fragments (half the L2 -> SM activation traffic and half the B-operand expansion); at T <= 32
+// only where that still leaves two CTAs per SM (measured: at N = 4096 the halved grid of 128 CTAs
+// costs more than the sharing saves there, and less at T = 64).
 template <bool ASYM>
-cudaError_t launch_asym(const DecodeParams& p, cudaStream_t stream) {
-  if (p.T <= 8) return launch_nt<1, ASYM>(p, stream);
-  if (p.T <= 16) return launch_nt<2, ASYM>(p, stream);
-  if (p.T <= 32) return launch_nt<4, ASYM>(p, stream);
-  return launch_nt<8, ASYM>(p, stream);
+cudaError_t launch_asym(const DecodeParams& p, int num_sms, cudaStream_t stream) {
+  if (p.T <= 8) return launch_nt<1, 1, ASYM>(p, stream);
+  if (p.T <= 16) return launch_nt<2, 1, ASYM>(p, stream);
+  const bool wide = p.N >= 2 * kRows * 2 * num_sms;
+  if (p.T <= 32) return wide ? launch_nt<4, 2, ASYM>(p, stream) : launch_nt<4, 1, ASYM>(p, stream);
+  return launch_nt<8, 2, ASYM>(p, stream);
 }
 
 }  // namespace
@@ -189,7 +241,7 @@ cudaError_t launch_w4a4_decode(const GemmLaunch& g) {
   if (g.x != nullptr || g.T > kDecodeMaxT) return cudaErrorNotSupported;
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
-  static_assert(kTileRows % kRows == 0, "a 16-row group must not straddle two weight boxes");
+  static_assert(kTileRows % (2 * kRows) == 0, "a CTA's row groups must not straddle two weight boxes");
   DecodeParams p{};
   p.tiles = base + h.off_tiles;
   p.sw = reinterpret_cast<const float*>(base + h.off_sw);
@@ -205,7 +257,8 @@ cudaError_t launch_w4a4_decode(const GemmLaunch& g) {
   p.N = g.N;
   p.K = g.K;
   p.num_kb = g.K / kTileK;
-  return g.zeros != nullptr ? launch_asym<true>(p, g.stream) : launch_asym<false>(p, g.stream);
+  const int sms = g.num_sms > 0 ? g.num_sms : 148;
+  return g.zeros != nullptr ? launch_asym<true>(p, sms, g.stream) : launch_asym<false>(p, sms, g.stream);
 }
 
 }  // namespace baseq
