@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     linear,
     linear_fused,
     linear_host,
+    linear_host_scratch_bytes,
     pack_weights,
     quantize_act,
     quantize_act_asym,

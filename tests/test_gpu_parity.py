@@ -574,3 +574,26 @@ def test_decode_strided_output():
     torch.cuda.synchronize()
     assert torch.equal(buf[:, :N].contiguous().view(torch.int16), y_ref.view(torch.int16))
     assert torch.all(buf[:, N:] == -1.0)
+
+
+# ------------------------------------------------------------------------------- host-buffer entry
+@pytest.mark.parametrize("T", [16, 130])
+def test_linear_host_matches_oracle(T):
+    # baseq_linear_host (bench.py's e2e leg): pinned host X in, pinned host Y out, H2D / quantise /
+    # GEMM / D2H enqueued by the library; T = 16 takes the decode GEMM, T = 130 the tcgen05 one
+    rng = np.random.default_rng(900 + T)
+    K, N = 512, 264
+    x = rand_x(rng, T, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    W = _rand_w(rng, N, K)
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(b), dev(W["layer_bias"]))
+    params = bq.ActParams(0.9, 1.05, None, dev(b), 0)
+    x_host = torch.from_numpy(x.view(np.int16)).view(torch.bfloat16).pin_memory()
+    y_host = torch.zeros((T, N), dtype=torch.bfloat16).pin_memory()
+    scratch = torch.empty(bq.linear_host_scratch_bytes(T, N, K), dtype=torch.uint8, device="cuda")
+    bq.linear_host(x_host, params, pw, y_host, scratch)
+    torch.cuda.synchronize()
+    ref = oracle.linear(x, W["w_nibbles"], W["w_scale"], fb, 0.9, 1.05, None, b, 0)
+    assert np.array_equal(pw.fused_bias.cpu().numpy().view(np.uint32), fb.view(np.uint32))
+    assert np.array_equal(y_host.view(torch.int16).numpy().view(np.uint16), ref["y"])
