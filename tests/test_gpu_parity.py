@@ -561,19 +561,24 @@ def test_decode_matches_prefill_kernel_on_shared_rows():
 
 
 def test_decode_strided_output():
-    # ldy > N: the decode kernel writes only the N columns of each row
+    # ldy > N and guard rows around Y / acc_dump: the decode kernel writes only the T x N outputs
     rng = np.random.default_rng(77)
-    T, K, N = 12, 512, 136
-    x = rand_x(rng, T, K)
-    W = _rand_w(rng, N, K)
-    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None, dev(W["layer_bias"]))
-    codes, scales = bq.quantize_act(bf16_dev(x), bq.ActParams(0.9))
-    y_ref = bq.w4a4_gemm(codes, scales, pw)
-    buf = torch.full((T, 160), -1.0, dtype=torch.bfloat16, device="cuda")
-    bq.w4a4_gemm(codes, scales, pw, y=buf[:, :N])
-    torch.cuda.synchronize()
-    assert torch.equal(buf[:, :N].contiguous().view(torch.int16), y_ref.view(torch.int16))
-    assert torch.all(buf[:, N:] == -1.0)
+    K, N = 512, 136
+    for T in (3, 12, 30, 57):
+        x = rand_x(rng, T, K)
+        W = _rand_w(rng, N, K)
+        pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None, dev(W["layer_bias"]))
+        codes, scales = bq.quantize_act(bf16_dev(x), bq.ActParams(0.9))
+        acc_ref = torch.empty((T, N), dtype=torch.int32, device="cuda")
+        y_ref = bq.w4a4_gemm(codes, scales, pw, acc_dump=acc_ref)
+        buf = torch.full((T + 2, 160), -1.0, dtype=torch.bfloat16, device="cuda")
+        accbuf = torch.full((T + 2, N), -7, dtype=torch.int32, device="cuda")
+        bq.w4a4_gemm(codes, scales, pw, y=buf[1:T + 1, :N], acc_dump=accbuf[1:T + 1])
+        torch.cuda.synchronize()
+        assert torch.equal(buf[1:T + 1, :N].contiguous().view(torch.int16), y_ref.view(torch.int16))
+        assert torch.all(buf[1:T + 1, N:] == -1.0) and torch.all(buf[0] == -1.0) and torch.all(buf[T + 1] == -1.0)
+        assert torch.equal(accbuf[1:T + 1], acc_ref)
+        assert torch.all(accbuf[0] == -7) and torch.all(accbuf[T + 1] == -7)
 
 
 # ------------------------------------------------------------------------------- host-buffer entry
