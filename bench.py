@@ -480,15 +480,32 @@ def run_decode(args, bq, torch, plan, data, acts, layers, hbm_gbs):
 
     w_bytes = sum(sp.N * sp.K / 2 for _a, specs in plan for sp in specs)
     ncopy = int(280e6 // w_bytes) + 2
+    def pack_merged(act, specs):
+        # layers that share one quantised activation, packed as ONE weight matrix (output channels
+        # concatenated): one GEMM launch instead of len(specs)
+        Ws = [data["weights"][sp.name] for sp in specs]
+        lb = None
+        if any(W["layer_bias"] is not None for W in Ws):
+            lb = np.concatenate([W["layer_bias"] if W["layer_bias"] is not None
+                                 else np.zeros(sp.N, np.float32) for W, sp in zip(Ws, specs)])
+        return bq.pack_weights(dev(np.concatenate([W["w_nibbles"] for W in Ws])),
+                               dev(np.concatenate([W["w_scale"] for W in Ws])),
+                               dev(data["acts"][act]["b"]), None if lb is None else dev(lb))
+
     copies = [{sp.name: layers[sp.name]["pw"] for _a, specs in plan for sp in specs}]
-    for _ in range(ncopy - 1):
-        c = {}
+    for i in range(ncopy):
+        c = copies[0] if i == 0 else {}
         for act, specs in plan:
-            for sp in specs:
-                W = data["weights"][sp.name]
-                c[sp.name] = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(data["acts"][act]["b"]),
-                                             None if W["layer_bias"] is None else dev(W["layer_bias"]))
-        copies.append(c)
+            if i > 0:
+                for sp in specs:
+                    W = data["weights"][sp.name]
+                    c[sp.name] = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]),
+                                                 dev(data["acts"][act]["b"]),
+                                                 None if W["layer_bias"] is None else dev(W["layer_bias"]))
+            if len(specs) > 1:
+                c["merged:" + act] = pack_merged(act, specs)
+        if i > 0:
+            copies.append(c)
     torch.cuda.synchronize()
     out = []
     for Td in (1, 8, 16, 32, 64, 65):
@@ -499,14 +516,18 @@ def run_decode(args, bq, torch, plan, data, acts, layers, hbm_gbs):
                          torch.empty((Td,), dtype=torch.float32, device="cuda"))
             for sp in specs:
                 bufs[sp.name] = torch.empty((Td, sp.N), dtype=torch.bfloat16, device="cuda")
+            bufs["merged:" + act] = torch.empty((Td, sum(sp.N for sp in specs)), dtype=torch.bfloat16,
+                                                device="cuda")
 
         def step(k, mode):
             pws = copies[k % ncopy]
             for act, specs in plan:
                 x, codes, scales = bufs[act]
-                if mode != "gemms":
+                if mode in ("step", "quant"):
                     bq.quantize_act(x, acts[act]["params"], codes, scales)
-                if mode != "quant":
+                if mode == "merged" and len(specs) > 1:
+                    bq.w4a4_gemm(codes, scales, pws["merged:" + act], bufs["merged:" + act])
+                elif mode != "quant":
                     for sp in specs:
                         bq.w4a4_gemm(codes, scales, pws[sp.name], bufs[sp.name])
 
@@ -514,7 +535,7 @@ def run_decode(args, bq, torch, plan, data, acts, layers, hbm_gbs):
         # ~ 8 us per call), so the timed loop replays a CUDA graph of ncopy consecutive steps
         # (one per weight copy); the eager figure is kept beside it.
         res, eager = {}, {}
-        for mode in ("step", "gemms", "quant"):
+        for mode in ("step", "gemms", "quant", "merged"):
             for k in range(ncopy):
                 step(k, mode)
             torch.cuda.synchronize()
@@ -550,7 +571,8 @@ def run_decode(args, bq, torch, plan, data, acts, layers, hbm_gbs):
                     "step_ms": res["step"], "tokens_per_s": Td / (res["step"] * 1e-3),
                     "quantizers_ms": res["quant"], "gemms_ms": res["gemms"], "gemm_GB_per_s": gbs, "frac_of_measured_hbm": gbs / hbm_gbs,
                     "weight_copies_rotated": ncopy, "timed_as": "CUDA graph of %d steps" % ncopy,
-                    "eager_step_ms": eager["step"], "eager_gemms_ms": eager["gemms"]})
+                    "eager_step_ms": eager["step"], "eager_gemms_ms": eager["gemms"],
+                    "gemms_ms_shared_activation_layers_packed_as_one": res["merged"]})
     del copies
     return out
 
