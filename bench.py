@@ -508,7 +508,8 @@ def run_decode(args, bq, torch, plan, data, acts, layers, hbm_gbs):
             copies.append(c)
     torch.cuda.synchronize()
     out = []
-    for Td in (1, 8, 16, 32, 64, 65):
+    T_full = min(a["x"].shape[0] for a in acts.values())
+    for Td in (1, 8, 16, 32, 64, 65, T_full):        # T_full: the prefill step, for the packed-as-one figure
         bufs = {}
         for act, specs in plan:
             a = acts[act]
@@ -567,12 +568,15 @@ def run_decode(args, bq, torch, plan, data, acts, layers, hbm_gbs):
             del graph
         by = sum(sp.N * sp.K / 2 + Td * sp.K / 2 + 2.0 * Td * sp.N for _a, specs in plan for sp in specs)
         gbs = by / (res["gemms"] * 1e-3) / 1e9
+        ops = sum(2.0 * Td * sp.N * sp.K for _a, specs in plan for sp in specs)
         out.append({"T": Td, "kernel": "w4a4_decode_kernel" if Td <= 64 else "w4a4_gemm_kernel (tcgen05)",
                     "step_ms": res["step"], "tokens_per_s": Td / (res["step"] * 1e-3),
                     "quantizers_ms": res["quant"], "gemms_ms": res["gemms"], "gemm_GB_per_s": gbs, "frac_of_measured_hbm": gbs / hbm_gbs,
                     "weight_copies_rotated": ncopy, "timed_as": "CUDA graph of %d steps" % ncopy,
                     "eager_step_ms": eager["step"], "eager_gemms_ms": eager["gemms"],
-                    "gemms_ms_shared_activation_layers_packed_as_one": res["merged"]})
+                    "gemms_ms_shared_activation_layers_packed_as_one": res["merged"],
+                    "gemm_TOP_per_s": ops / (res["gemms"] * 1e-3) / 1e12,
+                    "gemm_TOP_per_s_packed_as_one": ops / (res["merged"] * 1e-3) / 1e12})
     del copies
     return out
 
