@@ -125,19 +125,47 @@ __global__ void __launch_bounds__(kWarps * 32, NT == 1 ? 3 : (NT * MT <= 8 ? 2 :
   ptx::griddep_launch_dependents();
   ptx::griddep_wait();
 
+  // per-token epilogue operands, requested with the first activation fragments: their L2 round
+  // trip is over long before the partial sums meet
+  float st[kOut], zt[kOut];
+#pragma unroll
+  for (int i = 0; i < kOut; ++i) {
+    const int tok = tok0 + i * (kThreads / kCh);
+    st[i] = tok < p.T ? p.scales[tok] : 0.0f;
+    zt[i] = (ASYM && tok < p.T) ? p.zeros[tok] : 0.0f;
+  }
+
+  // T <= 16: the activation fragments travel with the window (one or two vectors per k-block), so
+  // a k-block's MMAs never wait for an L2 round trip of their own; larger T loads them per k-block
+  // (8 NT registers each)
+  constexpr bool kXPre = NT <= 2;
+  uint4 xs[kXPre ? kDepth : 1][NT];
+  auto load_x = [&](uint4 (&dst)[NT], int it) {
+#pragma unroll
+    for (int j = 0; j < NT; ++j) {
+      dst[j] = make_uint4(0, 0, 0, 0);
+      if (j * 8 + g < p.T)
+        dst[j] = ptx::ldg_nc(reinterpret_cast<const uint4*>(
+            xrow + static_cast<size_t>(j) * 8 * (p.K / 2) + (warp + it * kWarps) * 64));
+    }
+  };
+  if (kXPre) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d)
+      if (d < count) load_x(xs[kXPre ? d : 0], d);
+  }
+
   for (int base = 0; base < count; base += kDepth) {
 #pragma unroll
     for (int d = 0; d < kDepth; ++d) {
       const int it = base + d;
       if (it < count) {
-        const int kb = warp + it * kWarps;
         uint4 xa[NT];
+        if (kXPre) {
 #pragma unroll
-        for (int j = 0; j < NT; ++j) {
-          xa[j] = make_uint4(0, 0, 0, 0);
-          if (j * 8 + g < p.T)
-            xa[j] = ptx::ldg_nc(reinterpret_cast<const uint4*>(
-                xrow + static_cast<size_t>(j) * 8 * (p.K / 2) + kb * 64));
+          for (int j = 0; j < NT; ++j) xa[j] = xs[kXPre ? d : 0][j];
+        } else {
+          load_x(xa, it);
         }
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -160,18 +188,12 @@ __global__ void __launch_bounds__(kWarps * 32, NT == 1 ? 3 : (NT * MT <= 8 ? 2 :
             for (int m = 0; m < MT; ++m) mma_s8(acc[m][j], a0[m], a1[m], a2[m], a3[m], b0, b1);
           }
         }
-        if (it + kDepth < count) load_w(d, it + kDepth);
+        if (it + kDepth < count) {
+          load_w(d, it + kDepth);
+          if (kXPre) load_x(xs[kXPre ? d : 0], it + kDepth);
+        }
       }
     }
-  }
-
-  // per-token epilogue operands, requested before the partial sums meet
-  float st[kOut], zt[kOut];
-#pragma unroll
-  for (int i = 0; i < kOut; ++i) {
-    const int tok = tok0 + i * (kThreads / kCh);
-    st[i] = tok < p.T ? p.scales[tok] : 0.0f;
-    zt[i] = (ASYM && tok < p.T) ? p.zeros[tok] : 0.0f;
   }
 
   // the kWarps partial sums meet in shared memory (integer adds: any order, same result)
