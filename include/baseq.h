@@ -12,11 +12,13 @@
  * Conventions (all entry points)
  *  - plain C, no torch / C++ types; every pointer is a DEVICE pointer owned by the caller
  *    unless the argument name ends in _host;
- *  - the library never allocates, frees or synchronises, and keeps no reference to any
- *    argument after the call returns; all work is enqueued on `stream` (a cudaStream_t
- *    passed as void*; NULL = the legacy default stream);
- *  - arguments are validated on the host before anything is launched; every call returns a
- *    baseq_status_t (no exceptions, no errno, nothing printed);
+ *  - the library never allocates, frees or synchronises (baseq_sync_status is the one call that
+ *    blocks), and keeps no reference to any argument after the call returns; all work is enqueued
+ *    on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream);
+ *  - arguments are validated on the host before anything is launched or copied -- a call that
+ *    returns an error has enqueued nothing; every call returns a baseq_status_t (no exceptions,
+ *    no errno, nothing printed);
+ *  - any host thread may call, with any device current (one process may drive several GPUs);
  *  - there is no CPU fallback: on a device that is not compute capability 10.x every compute
  *    entry point returns BASEQ_ERR_UNSUPPORTED;
  *  - CUDA launch failures are returned as BASEQ_ERR_CUDA by the enqueueing call;
@@ -24,8 +26,9 @@
  *  - non-finite activations: behaviour unspecified (S:32 rejects them at construction).
  *
  * Shape rules (BASEQ_ERR_SHAPE): T >= 1 (empty input is an error, S:57 / S:225),
- * K % 128 == 0 and 128 <= K <= 32768 (a whole row stays in one CTA's registers),
- * N % 8 == 0 and N >= 8.  T need not be a multiple of any tile.
+ * K % 128 == 0 and 128 <= K <= 32768 in EVERY entry point (a whole row stays in one CTA; the GEMM's
+ * raw accumulator 256 * acc stays inside int32), N % 8 == 0 and N >= 8.  T need not be a multiple
+ * of any tile.
  * Alignment (BASEQ_ERR_ALIGN): x, codes, y, packed blob 16-byte aligned (blob: 128);
  * ldx >= K, ldx % 8 == 0; ldy >= N, ldy % 8 == 0.
  */
@@ -51,8 +54,9 @@ typedef enum {
   BASEQ_ERR_SHAPE = 2,       /* T/K/N violate the shape rules above                      */
   BASEQ_ERR_ALIGN = 3,       /* pointer or leading-dimension alignment                   */
   BASEQ_ERR_PARAM = 4,       /* alpha / gamma / had_block out of range                   */
-  BASEQ_ERR_WORKSPACE = 5,   /* workspace too small or blob header invalid               */
-  BASEQ_ERR_UNSUPPORTED = 6, /* not an sm_100 device                                     */
+  BASEQ_ERR_WORKSPACE = 5,   /* workspace / scratch too small; from baseq_sync_status: a
+                                packed blob did not match the (N, K) of a GEMM call       */
+  BASEQ_ERR_UNSUPPORTED = 6, /* not an sm_100 device, or a combination that is not built */
   BASEQ_ERR_CUDA = 7         /* a CUDA runtime / driver call failed                      */
 } baseq_status_t;
 
@@ -60,6 +64,13 @@ typedef enum {
 BASEQ_API const char* baseq_status_string(baseq_status_t s);
 /* Library version (integer, increases with ABI changes). */
 BASEQ_API int baseq_version(void);
+/* The one blocking call: synchronises `stream`, then reads and clears the current device's status
+ * word.  A packed blob lives in device memory, so no enqueue-only call can compare its header
+ * with the (N, K) it is given; the GEMM kernels do (magic, N, K -- written by baseq_pack_weights):
+ * on a mismatch the kernel does no work, writes nothing, and raises the word.  Returns
+ * BASEQ_ERR_WORKSPACE if any GEMM of this device since the last call found such a blob,
+ * BASEQ_ERR_CUDA if the synchronisation reports an asynchronous fault, else BASEQ_OK. */
+BASEQ_API baseq_status_t baseq_sync_status(void* stream);
 
 /* The per-quantizer parameters of Eq. 15 / BlockParams.
  *   u_k = g_k * h_k - b_k,  h = block-Hadamard(x) or x,  g_k = sa ? sa[k] : gamma    (C-1, C-2)
@@ -85,7 +96,14 @@ typedef struct {
  *   layer_bias  [N] fp32 or NULL
  *   packed_out  caller buffer of baseq_packed_weight_bytes(N, K) bytes, 128-byte aligned
  *   fused_bias_out  optional [N] copy of fb for inspection, or NULL
- * The blob is opaque, position independent (may be copied) and a pure function of the inputs. */
+ * The blob is opaque, position independent (may be copied) and a pure function of the inputs.
+ * Ordering: the GEMM kernels are enqueued with the programmatic-dependent-launch attribute and
+ * read the blob's header and weight boxes BEFORE they wait for the preceding kernel of the stream.
+ * Blobs written by baseq_pack_weights are safe by construction (header and boxes are followed by
+ * a fully serialised kernel boundary inside the call; s_w / fb / wsum, which its last kernel and
+ * baseq_set_fused_bias write, are read after the wait).  A blob the caller copies must be
+ * complete in stream order through a memcpy or a plain kernel launch, not through a kernel that
+ * triggers its dependents early. */
 BASEQ_API size_t baseq_packed_weight_bytes(int N, int K);
 BASEQ_API baseq_status_t baseq_pack_weights(const uint8_t* w_nibbles, const float* w_scale, const float* b,
                                   const float* layer_bias, int N, int K, void* packed_out,

@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     quantize_act_asym,
     w4a4_gemm_asym,
     quantize_kv,
+    sync_status,
     w4a4_gemm,
     EXPORTED_SYMBOLS,
 )

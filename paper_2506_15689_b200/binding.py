@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libbaseq.so")
 _lib = None
 
 EXPORTED_SYMBOLS = [
-    "baseq_status_string", "baseq_version", "baseq_packed_weight_bytes", "baseq_pack_weights",
+    "baseq_status_string", "baseq_version", "baseq_sync_status", "baseq_packed_weight_bytes", "baseq_pack_weights",
     "baseq_set_fused_bias", "baseq_quantize_act", "baseq_w4a4_gemm",
     "baseq_fused_workspace_bytes", "baseq_linear_fused", "baseq_linear_host_scratch_bytes",
     "baseq_linear_host", "baseq_quantize_act_asym", "baseq_w4a4_gemm_asym", "baseq_quantize_kv",
@@ -49,6 +49,8 @@ def lib():
         L.baseq_status_string.argtypes = [i32]
         L.baseq_version.restype = i32
         L.baseq_version.argtypes = []
+        L.baseq_sync_status.restype = i32
+        L.baseq_sync_status.argtypes = [vp]
         L.baseq_packed_weight_bytes.restype = sz
         L.baseq_packed_weight_bytes.argtypes = [i32, i32]
         L.baseq_pack_weights.restype = i32
@@ -89,6 +91,12 @@ def _p(t):
 def _check(status, where):
     if status != 0:
         raise BaseqError(status, where)
+
+
+def sync_status():
+    """Synchronises the current stream and raises BaseqError(BASEQ_ERR_WORKSPACE) if a GEMM since the
+    last call found a packed blob that does not match its (N, K)."""
+    _check(lib().baseq_sync_status(_stream()), "baseq_sync_status")
 
 
 class ActParams:

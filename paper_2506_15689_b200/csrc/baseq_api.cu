@@ -2,6 +2,7 @@
 // No compute happens here and nothing falls back to the CPU.
 #include <cmath>
 #include <cstring>
+#include <mutex>
 
 #include "../../include/baseq.h"
 #include "kernels.cuh"
@@ -10,36 +11,62 @@ namespace {
 
 using namespace baseq;
 
+// One word per device (a __device__ variable exists once per context): bit 0 is raised by a GEMM
+// kernel that finds a packed-weight header not matching its (N, K) arguments.
+__device__ unsigned int g_status_word;
+
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
-struct DeviceInfo {
-  bool ok = false;
-  bool queried = false;
+// Per-device state, filled once per device under std::call_once (any number of host threads, any
+// number of GPUs in one process): compute capability, SM count, and the address of this device's
+// copy of the library's status word (see baseq_sync_status).
+struct DeviceState {
+  std::once_flag once;
+  baseq_status_t st = BASEQ_ERR_CUDA;
   int num_sms = 0;
+  unsigned int* status_word = nullptr;
+};
+DeviceState g_dev[kMaxDevices];
+
+struct DeviceRef {
+  int device = 0;
+  int num_sms = 0;
+  unsigned int* status_word = nullptr;
 };
 
-// Cached per process for the current device at first use (one GPU per process).
-baseq_status_t device_check(int* num_sms) {
-  static DeviceInfo info;
-  if (!info.queried) {
-    int dev = 0, major = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return BASEQ_ERR_CUDA;
-    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess)
-      return BASEQ_ERR_CUDA;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-      return BASEQ_ERR_CUDA;
-    info.ok = (major == 10);
-    info.num_sms = sms;
-    info.queried = true;
+baseq_status_t device_check(DeviceRef* out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return BASEQ_ERR_CUDA;
+  if (dev < 0 || dev >= kMaxDevices) return BASEQ_ERR_UNSUPPORTED;
+  DeviceState& d = g_dev[dev];
+  std::call_once(d.once, [&d, dev]() {
+    int major = 0, sms = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return;
+    if (major != 10) {
+      d.st = BASEQ_ERR_UNSUPPORTED;
+      return;
+    }
+    void* sym = nullptr;
+    if (cudaGetSymbolAddress(&sym, g_status_word) != cudaSuccess) return;
+    d.status_word = static_cast<unsigned int*>(sym);
+    d.num_sms = sms;
+    d.st = BASEQ_OK;
+  });
+  if (d.st != BASEQ_OK) return d.st;
+  if (out) {
+    out->device = dev;
+    out->num_sms = d.num_sms;
+    out->status_word = d.status_word;
   }
-  if (!info.ok) return BASEQ_ERR_UNSUPPORTED;
-  if (num_sms) *num_sms = info.num_sms;
   return BASEQ_OK;
 }
 
+// K <= 32768 everywhere: a whole row stays in one CTA (quantiser), and the GEMM's raw accumulator
+// 256 * acc stays inside int32 (|256 * 64 * K| = 2^29 symmetric, |256 * 120 * K| < 2^30 asymmetric).
 baseq_status_t check_shape(int T, int N, int K) {
   if (T < 1) return BASEQ_ERR_SHAPE;
-  if (K < 128 || (K % 128) != 0) return BASEQ_ERR_SHAPE;
+  if (K < 128 || (K % 128) != 0 || K > kMaxK) return BASEQ_ERR_SHAPE;
   if (N < 8 || (N % 8) != 0) return BASEQ_ERR_SHAPE;
   return BASEQ_OK;
 }
@@ -76,10 +103,10 @@ QuantLaunch make_quant(const void* x, int64_t ldx, int T, int K, const baseq_act
   q.scales = scales;
   q.stream = static_cast<cudaStream_t>(stream);
   q.tpr_log2 = 0;
-  q.tpr_log2_override = 0;
   q.zeros = nullptr;
   q.asym = false;
   q.num_sms = 148;          // overwritten by the callers from the device query
+  q.device = 0;
   q.blocks_per_sm = 2;
   return q;
 }
@@ -92,20 +119,33 @@ const char* baseq_status_string(baseq_status_t s) {
   switch (s) {
     case BASEQ_OK: return "BASEQ_OK";
     case BASEQ_ERR_NULL: return "BASEQ_ERR_NULL: a required pointer is NULL";
-    case BASEQ_ERR_SHAPE: return "BASEQ_ERR_SHAPE: need T >= 1, K % 128 == 0, N % 8 == 0";
+    case BASEQ_ERR_SHAPE: return "BASEQ_ERR_SHAPE: need T >= 1, K % 128 == 0, 128 <= K <= 32768, N % 8 == 0";
     case BASEQ_ERR_ALIGN: return "BASEQ_ERR_ALIGN: pointer or leading dimension misaligned";
     case BASEQ_ERR_PARAM: return "BASEQ_ERR_PARAM: alpha / gamma / had_block out of range";
-    case BASEQ_ERR_WORKSPACE: return "BASEQ_ERR_WORKSPACE: workspace too small or blob invalid";
-    case BASEQ_ERR_UNSUPPORTED: return "BASEQ_ERR_UNSUPPORTED: requires an sm_100 (B200) device";
+    case BASEQ_ERR_WORKSPACE: return "BASEQ_ERR_WORKSPACE: workspace too small, or a packed blob did not match (N, K)";
+    case BASEQ_ERR_UNSUPPORTED: return "BASEQ_ERR_UNSUPPORTED: requires an sm_100 (B200) device, or the combination is not built";
     case BASEQ_ERR_CUDA: return "BASEQ_ERR_CUDA: a CUDA call failed";
   }
   return "BASEQ: unknown status";
 }
 
-int baseq_version(void) { return 1; }
+int baseq_version(void) { return 2; }
+
+baseq_status_t baseq_sync_status(void* stream) {
+  DeviceRef d;
+  const baseq_status_t st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  unsigned int word = 0;
+  if (cudaMemcpyAsync(&word, d.status_word, sizeof word, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+    return BASEQ_ERR_CUDA;
+  if (cudaMemsetAsync(d.status_word, 0, sizeof word, s) != cudaSuccess) return BASEQ_ERR_CUDA;
+  if (cudaStreamSynchronize(s) != cudaSuccess) return BASEQ_ERR_CUDA;
+  return (word & kStatusBadBlob) ? BASEQ_ERR_WORKSPACE : BASEQ_OK;
+}
 
 size_t baseq_packed_weight_bytes(int N, int K) {
-  if (N < 8 || (N % 8) != 0 || K < 128 || (K % 128) != 0) return 0;
+  if (check_shape(1, N, K) != BASEQ_OK) return 0;
   return blob_bytes(N, K);
 }
 
@@ -134,98 +174,43 @@ baseq_status_t baseq_set_fused_bias(void* packed, int N, int K, const float* fb,
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
 }
 
-baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int T, int K,
-                                  const baseq_act_params_t* p, uint8_t* codes, float* scales,
-                                  void* stream) {
+namespace {
+
+// Everything baseq_quantize_act / _asym check, without launching: shared with the entry points that
+// call them after having enqueued other work (fused, host), so that a failing call enqueues nothing.
+baseq_status_t validate_quant(const void* x, int64_t ldx, int T, int K, const baseq_act_params_t* p,
+                              const void* codes, const void* scales, bool need_codes) {
   baseq_status_t st = check_shape(T, 8, K);     // empty input is a shape error
   if (st != BASEQ_OK) return st;
-  if (x_bf16 == nullptr || codes == nullptr || scales == nullptr || p == nullptr)
+  if (x == nullptr || scales == nullptr || p == nullptr || (need_codes && codes == nullptr))
     return BASEQ_ERR_NULL;
-  if (K > quant_max_k()) return BASEQ_ERR_SHAPE;
   st = check_act_params(p, K);
   if (st != BASEQ_OK) return st;
-  if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4)) return BASEQ_ERR_ALIGN;
+  if (!aligned(x, 16) || !aligned(codes, 16) || !aligned(scales, 4)) return BASEQ_ERR_ALIGN;
   if (ldx < K || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;
-  int sms = 0;
-  st = device_check(&sms);
-  if (st != BASEQ_OK) return st;
-  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
-  q.num_sms = sms;
-  const cudaError_t e = launch_quantize_act(q, true);
-  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+  return BASEQ_OK;
 }
 
-baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const void* packed_w,
-                               int T, int N, int K, void* y_bf16, int64_t ldy, int32_t* acc_dump,
-                               void* stream) {
-  if (codes == nullptr || scales == nullptr || packed_w == nullptr || y_bf16 == nullptr)
+baseq_status_t validate_gemm(const void* codes, const void* scales, const void* packed_w, int T, int N,
+                             int K, const void* y, int64_t ldy, const void* acc_dump, bool need_codes) {
+  if ((need_codes && codes == nullptr) || scales == nullptr || packed_w == nullptr || y == nullptr)
     return BASEQ_ERR_NULL;
-  baseq_status_t st = check_shape(T, N, K);
+  const baseq_status_t st = check_shape(T, N, K);
   if (st != BASEQ_OK) return st;
-  if (K > 131072) return BASEQ_ERR_SHAPE;            // raw accumulator 256*acc must fit int32
-  if (!aligned(codes, 16) || !aligned(y_bf16, 16) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
+  if (!aligned(codes, 16) || !aligned(y, 16) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
   if (acc_dump != nullptr && !aligned(acc_dump, 16)) return BASEQ_ERR_ALIGN;
   if (ldy < N || (ldy % 8) != 0) return BASEQ_ERR_ALIGN;
-  int sms = 0;
-  st = device_check(&sms);
-  if (st != BASEQ_OK) return st;
-  GemmLaunch g{};
-  g.codes = codes;
-  g.scales = scales;
-  g.blob = packed_w;
-  g.T = T;
-  g.N = N;
-  g.K = K;
-  g.y = y_bf16;
-  g.ldy = ldy;
-  g.acc_dump = acc_dump;
-  g.stream = static_cast<cudaStream_t>(stream);
-  g.num_sms = sms;
-  const cudaError_t e = launch_w4a4_gemm(g);
+  return BASEQ_OK;
+}
+
+baseq_status_t from_cuda(cudaError_t e) {
   if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
   return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
 }
 
-baseq_status_t baseq_quantize_act_asym(const void* x_bf16, int64_t ldx, int T, int K,
-                                       const baseq_act_params_t* p, uint8_t* codes, float* scales,
-                                       float* zeros, void* stream) {
-  baseq_status_t st = check_shape(T, 8, K);
-  if (st != BASEQ_OK) return st;
-  if (x_bf16 == nullptr || codes == nullptr || scales == nullptr || zeros == nullptr || p == nullptr)
-    return BASEQ_ERR_NULL;
-  if (K > quant_max_k()) return BASEQ_ERR_SHAPE;
-  st = check_act_params(p, K);
-  if (st != BASEQ_OK) return st;
-  if (p->sa != nullptr) return BASEQ_ERR_UNSUPPORTED;
-  if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4) || !aligned(zeros, 4))
-    return BASEQ_ERR_ALIGN;
-  if (ldx < K || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;
-  int sms = 0;
-  st = device_check(&sms);
-  if (st != BASEQ_OK) return st;
-  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
-  q.num_sms = sms;
-  q.zeros = zeros;
-  q.asym = true;
-  const cudaError_t e = launch_quantize_ring(q, true);
-  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
-}
-
-baseq_status_t baseq_w4a4_gemm_asym(const uint8_t* codes, const float* scales, const float* zeros,
-                                    const void* packed_w, int T, int N, int K, void* y_bf16,
-                                    int64_t ldy, int32_t* acc_dump, void* stream) {
-  if (codes == nullptr || scales == nullptr || zeros == nullptr || packed_w == nullptr ||
-      y_bf16 == nullptr)
-    return BASEQ_ERR_NULL;
-  baseq_status_t st = check_shape(T, N, K);
-  if (st != BASEQ_OK) return st;
-  if (K > 65536) return BASEQ_ERR_SHAPE;             // raw accumulator 256 * 120 * K must fit int32
-  if (!aligned(codes, 16) || !aligned(y_bf16, 16) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
-  if (acc_dump != nullptr && !aligned(acc_dump, 16)) return BASEQ_ERR_ALIGN;
-  if (ldy < N || (ldy % 8) != 0) return BASEQ_ERR_ALIGN;
-  int sms = 0;
-  st = device_check(&sms);
-  if (st != BASEQ_OK) return st;
+GemmLaunch make_gemm(const uint8_t* codes, const float* scales, const float* zeros, const void* packed_w,
+                     int T, int N, int K, void* y, int64_t ldy, int32_t* acc_dump, void* stream,
+                     const DeviceRef& d) {
   GemmLaunch g{};
   g.codes = codes;
   g.scales = scales;
@@ -234,14 +219,73 @@ baseq_status_t baseq_w4a4_gemm_asym(const uint8_t* codes, const float* scales, c
   g.T = T;
   g.N = N;
   g.K = K;
-  g.y = y_bf16;
+  g.y = y;
   g.ldy = ldy;
   g.acc_dump = acc_dump;
   g.stream = static_cast<cudaStream_t>(stream);
-  g.num_sms = sms;
-  const cudaError_t e = launch_w4a4_gemm(g);
-  if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
-  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+  g.num_sms = d.num_sms;
+  g.device = d.device;
+  g.status_word = d.status_word;
+  return g;
+}
+
+}  // namespace
+
+baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int T, int K,
+                                  const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                  void* stream) {
+  baseq_status_t st = validate_quant(x_bf16, ldx, T, K, p, codes, scales, true);
+  if (st != BASEQ_OK) return st;
+  DeviceRef d;
+  st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
+  q.num_sms = d.num_sms;
+  q.device = d.device;
+  return from_cuda(launch_quantize_act(q, true));
+}
+
+baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const void* packed_w,
+                               int T, int N, int K, void* y_bf16, int64_t ldy, int32_t* acc_dump,
+                               void* stream) {
+  baseq_status_t st = validate_gemm(codes, scales, packed_w, T, N, K, y_bf16, ldy, acc_dump, true);
+  if (st != BASEQ_OK) return st;
+  DeviceRef d;
+  st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  return from_cuda(launch_w4a4_gemm(
+      make_gemm(codes, scales, nullptr, packed_w, T, N, K, y_bf16, ldy, acc_dump, stream, d)));
+}
+
+baseq_status_t baseq_quantize_act_asym(const void* x_bf16, int64_t ldx, int T, int K,
+                                       const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                       float* zeros, void* stream) {
+  baseq_status_t st = validate_quant(x_bf16, ldx, T, K, p, codes, scales, true);
+  if (st != BASEQ_OK) return st;
+  if (zeros == nullptr) return BASEQ_ERR_NULL;
+  if (!aligned(zeros, 4)) return BASEQ_ERR_ALIGN;
+  DeviceRef d;
+  st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
+  q.num_sms = d.num_sms;
+  q.device = d.device;
+  q.zeros = zeros;
+  q.asym = true;
+  return from_cuda(launch_quantize_act(q, true));
+}
+
+baseq_status_t baseq_w4a4_gemm_asym(const uint8_t* codes, const float* scales, const float* zeros,
+                                    const void* packed_w, int T, int N, int K, void* y_bf16,
+                                    int64_t ldy, int32_t* acc_dump, void* stream) {
+  if (zeros == nullptr) return BASEQ_ERR_NULL;
+  baseq_status_t st = validate_gemm(codes, scales, packed_w, T, N, K, y_bf16, ldy, acc_dump, true);
+  if (st != BASEQ_OK) return st;
+  DeviceRef d;
+  st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  return from_cuda(launch_w4a4_gemm(
+      make_gemm(codes, scales, zeros, packed_w, T, N, K, y_bf16, ldy, acc_dump, stream, d)));
 }
 
 baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int T, int n_heads, int head_dim,
@@ -255,8 +299,8 @@ baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int T, int n_h
   if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4) || !aligned(zeros, 4))
     return BASEQ_ERR_ALIGN;
   if (ldx < static_cast<int64_t>(n_heads) * head_dim || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;
-  int sms = 0;
-  const baseq_status_t st = device_check(&sms);
+  DeviceRef d;
+  const baseq_status_t st = device_check(&d);
   if (st != BASEQ_OK) return st;
   KvLaunch q{};
   q.x = x_bf16;
@@ -268,18 +312,14 @@ baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int T, int n_h
   q.codes = codes;
   q.scales = scales;
   q.zeros = zeros;
-  q.num_sms = sms;
+  q.num_sms = d.num_sms;
   q.stream = static_cast<cudaStream_t>(stream);
-  const cudaError_t e = launch_quantize_kv(q);
-  if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
-  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+  return from_cuda(launch_quantize_kv(q));
 }
 
 size_t baseq_fused_workspace_bytes(int T, int N, int K) {
-  (void)N;
-  (void)K;
-  if (T < 1) return 0;
-  return 256;   // the fused path keeps everything on chip; a small fixed scratch is reserved
+  if (check_shape(T, N, K) != BASEQ_OK) return 0;
+  return fused_workspace_bytes(T, N, K);
 }
 
 baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
@@ -287,37 +327,22 @@ baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
                                   void* y_bf16, int64_t ldy, void* workspace, size_t workspace_bytes,
                                   uint8_t* codes_dump, float* scales_out, int32_t* acc_dump,
                                   void* stream) {
-  if (x_bf16 == nullptr || p == nullptr || packed_w == nullptr || y_bf16 == nullptr ||
-      scales_out == nullptr || workspace == nullptr)
-    return BASEQ_ERR_NULL;
-  baseq_status_t st = check_shape(T, N, K);
+  // every check of both stages first: a failing call enqueues nothing
+  if (workspace == nullptr) return BASEQ_ERR_NULL;
+  baseq_status_t st = validate_quant(x_bf16, ldx, T, K, p, codes_dump, scales_out, false);
   if (st != BASEQ_OK) return st;
-  if (K > quant_max_k()) return BASEQ_ERR_SHAPE;
-  st = check_act_params(p, K);
+  st = validate_gemm(nullptr, scales_out, packed_w, T, N, K, y_bf16, ldy, acc_dump, false);
   if (st != BASEQ_OK) return st;
-  if (!aligned(x_bf16, 16) || !aligned(y_bf16, 16) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
-  if (ldx < K || (ldx % 8) != 0 || ldy < N || (ldy % 8) != 0) return BASEQ_ERR_ALIGN;
+  if (!aligned(workspace, 256)) return BASEQ_ERR_ALIGN;
   if (workspace_bytes < baseq_fused_workspace_bytes(T, N, K)) return BASEQ_ERR_WORKSPACE;
-  int sms = 0;
-  st = device_check(&sms);
+  if (!fused_supported(p->had_block)) return BASEQ_ERR_UNSUPPORTED;
+  DeviceRef d;
+  st = device_check(&d);
   if (st != BASEQ_OK) return st;
-  // pass 1: per-token absmax -> scales (reads X once, writes T floats)
-  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, nullptr, scales_out, stream);
-  q.num_sms = sms;
-  cudaError_t e = launch_quantize_act(q, false);
-  if (e != cudaSuccess) return BASEQ_ERR_CUDA;
-  // pass 2: GEMM with the quantise-in-producer variant
-  GemmLaunch g{};
-  g.scales = scales_out;
-  g.blob = packed_w;
-  g.T = T;
-  g.N = N;
-  g.K = K;
-  g.y = y_bf16;
-  g.ldy = ldy;
-  g.acc_dump = acc_dump;
+  GemmLaunch g = make_gemm(nullptr, scales_out, nullptr, packed_w, T, N, K, y_bf16, ldy, acc_dump, stream, d);
   g.x = x_bf16;
   g.ldx = ldx;
+  g.alpha = p->alpha;
   g.gamma = p->gamma;
   g.sa = p->sa;
   g.b = p->b;
@@ -326,15 +351,12 @@ baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
                     ? static_cast<float>(1.0 / std::sqrt(static_cast<double>(p->had_block)))
                     : 1.0f;
   g.codes_dump = codes_dump;
-  g.stream = static_cast<cudaStream_t>(stream);
-  g.num_sms = sms;
-  e = launch_w4a4_gemm(g);
-  if (e == cudaErrorNotSupported) return BASEQ_ERR_UNSUPPORTED;
-  return e == cudaSuccess ? BASEQ_OK : BASEQ_ERR_CUDA;
+  g.workspace = workspace;
+  return from_cuda(launch_linear_fused(g));
 }
 
 size_t baseq_linear_host_scratch_bytes(int T, int N, int K) {
-  if (T < 1 || N < 8 || K < 128) return 0;
+  if (check_shape(T, N, K) != BASEQ_OK) return 0;
   auto up = [](size_t v) { return (v + 255) / 256 * 256; };
   return up(static_cast<size_t>(T) * K * 2) + up(static_cast<size_t>(T) * K / 2) +
          up(static_cast<size_t>(T) * 4) + up(static_cast<size_t>(T) * N * 2);
@@ -349,13 +371,20 @@ baseq_status_t baseq_linear_host(const void* x_bf16_host, int T, int K, const ba
   baseq_status_t st = check_shape(T, N, K);
   if (st != BASEQ_OK) return st;
   if (dev_scratch_bytes < baseq_linear_host_scratch_bytes(T, N, K)) return BASEQ_ERR_WORKSPACE;
-  if (!aligned(dev_scratch, 256)) return BASEQ_ERR_ALIGN;
+  if (!aligned(dev_scratch, 256) || !aligned(packed_w, 128)) return BASEQ_ERR_ALIGN;
   auto up = [](size_t v) { return (v + 255) / 256 * 256; };
   uint8_t* base = static_cast<uint8_t*>(dev_scratch);
   void* dx = base;
   uint8_t* dcodes = base + up(static_cast<size_t>(T) * K * 2);
   float* dscales = reinterpret_cast<float*>(dcodes + up(static_cast<size_t>(T) * K / 2));
   void* dy = reinterpret_cast<uint8_t*>(dscales) + up(static_cast<size_t>(T) * 4);
+  // every check of the two nested calls before the first copy is enqueued
+  st = validate_quant(dx, K, T, K, p, dcodes, dscales, true);
+  if (st != BASEQ_OK) return st;
+  st = validate_gemm(dcodes, dscales, packed_w, T, N, K, dy, N, nullptr, true);
+  if (st != BASEQ_OK) return st;
+  st = device_check(nullptr);
+  if (st != BASEQ_OK) return st;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (cudaMemcpyAsync(dx, x_bf16_host, static_cast<size_t>(T) * K * 2, cudaMemcpyHostToDevice, s) !=
       cudaSuccess)

@@ -1,10 +1,29 @@
 // Internal launch interfaces between baseq_api.cu and the kernel translation units.
 #pragma once
+#include <atomic>
 #include <cstddef>
 #include <cstdint>
 #include <cuda_runtime.h>
 
 namespace baseq {
+
+constexpr int kMaxDevices = 64;        // per-device host state (attributes set, status word) is indexed by device
+constexpr int kMaxK = 32768;           // library-wide bound on K (include/baseq.h, shape rules)
+constexpr unsigned int kStatusBadBlob = 1u;   // status-word bit: a GEMM found a blob header != its (N, K)
+
+// Raises a kernel's dynamic shared-memory limit once per device (thread-safe; setting the attribute
+// twice from two racing threads is harmless).  `slots` is one zero-initialised array per kernel.
+template <typename Kern>
+inline cudaError_t ensure_dynamic_smem(Kern kern, int bytes, int device, std::atomic<int>* slots) {
+  if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+  if (slots[device].load(std::memory_order_acquire) >= bytes) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return e;
+  int cur = slots[device].load(std::memory_order_relaxed);
+  while (cur < bytes && !slots[device].compare_exchange_weak(cur, bytes, std::memory_order_release)) {
+  }
+  return cudaSuccess;
+}
 
 // ------------------------------------------------------------------ packed weight blob
 // [ header 128 B | s_w[Npad] f32 | fb[Npad] f32 | wsum[Npad] f32 | boxes ]
@@ -63,11 +82,10 @@ struct QuantLaunch {
   bool asym;           // NEXT-1: per-token asymmetric int4 (unsigned codes)
   cudaStream_t stream;
   int tpr_log2;            // filled by the launcher
-  int tpr_log2_override;   // 0 = heuristic (tuning hook for profiling runs)
   int num_sms;             // persistent grid = num_sms * blocks_per_sm
+  int device;              // current device ordinal (per-device attribute cache)
   int blocks_per_sm;
 };
-int quant_max_k();
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes);
 // long rows (K >= 4096): bulk-TMA ring variant of the same contract (quantize_ring.cu)
 bool quantize_ring_supported(int K);
@@ -107,17 +125,24 @@ struct GemmLaunch {
   // fused producer inputs (x != nullptr selects the quantise-in-producer variant)
   const void* x;
   int64_t ldx;
-  float gamma;
+  float alpha, gamma;
   const float* sa;
   const float* b;
   int had_block;
   float had_scale;
   uint8_t* codes_dump;     // optional [T, K/2]
+  void* workspace;         // fused variant: baseq_fused_workspace_bytes(T, N, K) bytes
   cudaStream_t stream;
   int num_sms;
+  int device;              // current device ordinal
+  unsigned int* status_word;   // this device's status word (kStatusBadBlob)
 };
 // Returns cudaSuccess, or an error (cudaErrorNotSupported when the tensor map cannot be built).
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g);
+// Fused variant (a10): scales pre-pass + quantise-in-producer GEMM; g.x != nullptr, g.scales = scales_out.
+size_t fused_workspace_bytes(int T, int N, int K);
+bool fused_supported(int had_block);
+cudaError_t launch_linear_fused(const GemmLaunch& g);
 // Decode shapes (NEXT-4, w4a4_decode.cu): the same contract and the same bits for T <= kDecodeMaxT,
 // bound by streaming the packed weights once; launch_w4a4_gemm routes the unfused calls there.
 constexpr int kDecodeMaxT = 64;

@@ -182,14 +182,15 @@ cudaError_t launch_hw(const QuantLaunch& q, int V) {
 
 }  // namespace
 
-int quant_max_k() { return 512 * kMaxV * 8; }
+static_assert(512 * kMaxV * 8 >= kMaxK, "a row of kMaxK channels fits 512 threads x kMaxV vectors");
 
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes) {
+  // the asymmetric variant (NEXT-1) lives in the ring kernels only, scalar s^a
+  if (q.asym) return q.sa != nullptr ? cudaErrorNotSupported : launch_quantize_ring(q, write_codes);
   // long rows with the scalar s^a (every benchmark shape): bulk-TMA ring kernel; a per-channel
   // s^a vector takes the ring's split kernel at K = 4096 and the register-resident kernel below
   // otherwise
-  if (quantize_ring_supported(q.K) && q.tpr_log2_override == 0 &&
-      (q.sa == nullptr || quantize_ring_supports_sa(q.K, q.had_block)))
+  if (quantize_ring_supported(q.K) && (q.sa == nullptr || quantize_ring_supports_sa(q.K, q.had_block)))
     return launch_quantize_ring(q, write_codes);
   const int nvec = q.K / 8;
   // smallest power-of-two threads-per-row (>= 32) with at most 4 vectors per thread (the fp32 row
@@ -198,9 +199,6 @@ cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes) {
   int tl = 5;
   while (tl < 9 && ((nvec + (1 << tl) - 1) >> tl) > 4) ++tl;
   if (((nvec + (1 << tl) - 1) >> tl) > kMaxV) return cudaErrorInvalidValue;
-  if (q.tpr_log2_override >= 5 && q.tpr_log2_override <= 9 &&
-      ((nvec + (1 << q.tpr_log2_override) - 1) >> q.tpr_log2_override) <= kMaxV)
-    tl = q.tpr_log2_override;
   q.tpr_log2 = tl;
   const int V = (nvec + (1 << tl) - 1) >> tl;
   if (q.had_block) {

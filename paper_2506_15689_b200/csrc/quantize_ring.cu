@@ -449,13 +449,9 @@ cudaError_t launch_ring_split(const QuantLaunch& q) {
   p.stages = stages > kMaxStages ? kMaxStages : stages;
   if (p.stages < 2) return cudaErrorInvalidValue;
   const int smem = p.stages * p.stage_bytes + sa_bytes;
-  static int attr_smem = 0;
-  if (smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(quantize_ring_split_kernel<V, WC, ASYM, SA>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_smem = smem;
-  }
+  static std::atomic<int> attr_smem[kMaxDevices];
+  const cudaError_t ea = ensure_dynamic_smem(quantize_ring_split_kernel<V, WC, ASYM, SA>, smem, q.device, attr_smem);
+  if (ea != cudaSuccess) return ea;
   const int groups = (q.T + kSplitGroups - 1) / kSplitGroups;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
   return launch_pdl(quantize_ring_split_kernel<V, WC, ASYM, SA>, blocks, kRingThreads, smem, q.stream, p);
@@ -482,13 +478,9 @@ cudaError_t launch_ring_a(const QuantLaunch& q) {
   p.stages = stages > kMaxStages ? kMaxStages : stages;
   if (p.stages < 2) return cudaErrorInvalidValue;
   const int smem = p.stages * p.stage_bytes;
-  static int attr_smem = 0;
-  if (smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_smem = smem;
-  }
+  static std::atomic<int> attr_smem[kMaxDevices];
+  const cudaError_t ea = ensure_dynamic_smem(quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM>, smem, q.device, attr_smem);
+  if (ea != cudaSuccess) return ea;
   const int groups = (q.T + RL - 1) / RL;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
   return launch_pdl(quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM>, blocks, kRingThreads, smem, q.stream, p);

@@ -33,6 +33,8 @@ namespace {
 constexpr int kRows = 16;          // output channels per CTA (MMA M)
 
 struct DecodeParams {
+  const uint32_t* header;   // blob header: magic, N, K, ... (checked against N, K)
+  unsigned int* status;     // device status word
   const uint8_t* tiles;
   const float* sw;
   const float* fb;
@@ -79,13 +81,12 @@ __global__ void __launch_bounds__(kWarps * 32, NT == 1 ? 3 : (NT * MT <= 8 ? 2 :
       (static_cast<size_t>(n0 / kTileRows) * p.num_kb * kTileRows + (n0 % kTileRows) + g) * 64 + t4 * 16;
   const uint8_t* xrow = p.codes + static_cast<size_t>(g) * (p.K / 2) + t4 * 16;
 
-  // epilogue: this thread's outputs are one channel (ch) x tokens tok0 + i * (kThreads / kCh); the
-  // per-channel operands come from the weight blob and are requested first
+  // epilogue: this thread's outputs are one channel (ch) x tokens tok0 + i * (kThreads / kCh)
   const int ch = threadIdx.x % kCh, tok0 = threadIdx.x / kCh;
   const int n = n0 + ch;
-  const bool n_ok = n < p.N;
-  const float sw = n_ok ? p.sw[n] : 0.0f, fb = n_ok ? p.fb[n] : 0.0f;
-  const float ws = (ASYM && n_ok) ? p.wsum[n] : 0.0f;
+  // requested with the first weight window, compared after the wait: a blob packed for another
+  // (N, K) makes the whole grid write nothing and raises the status word (as in w4a4_gemm.cu)
+  const uint4 hdr = ptx::ldg_nc(reinterpret_cast<const uint4*>(p.header));
   for (int i = threadIdx.x; i < MT * NT * 4 * 32; i += kThreads) red[i] = 0;
 
   int32_t acc[MT][NT][4];
@@ -118,12 +119,28 @@ __global__ void __launch_bounds__(kWarps * 32, NT == 1 ? 3 : (NT * MT <= 8 ? 2 :
     }
     if (d < count) load_w(d, d);
   }
-  // The first window of W is in flight.  Let the next kernel of the stream start on the SMs this
-  // grid leaves free (a following decode GEMM streams ITS weights meanwhile; every kernel of this
-  // library writes only after its own griddepcontrol.wait), then wait for the preceding kernel:
-  // codes and scales are its output.
+  // The first window of W is in flight.  Only the weight BOXES may be read up here: they are written
+  // by the packer's retile kernel, which is followed by a fully serialised kernel boundary inside
+  // baseq_pack_weights (its scales / fused-bias kernel is a plain launch), so they are complete and
+  // visible before any programmatically launched kernel can start.  s_w, fb and wsum are written by
+  // the LAST packer kernel and by baseq_set_fused_bias, possibly the direct predecessor of a
+  // quantiser that triggers its dependents early: they are read after griddepcontrol.wait.
+  // Let the next kernel of the stream start on the SMs this grid leaves free (a following decode
+  // GEMM streams ITS weights meanwhile; every kernel of this library writes only after its own
+  // griddepcontrol.wait), then wait for the preceding kernel: codes and scales are its output.
   ptx::griddep_launch_dependents();
   ptx::griddep_wait();
+
+  const bool blob_ok = hdr.x == kBlobMagic && hdr.y == static_cast<uint32_t>(p.N) &&
+                       hdr.z == static_cast<uint32_t>(p.K);
+  if (!blob_ok) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) atomicOr(p.status, kStatusBadBlob);
+    return;
+  }
+  const bool n_ok = n < p.N;
+  // per-channel epilogue operands from the blob header area
+  const float sw = n_ok ? p.sw[n] : 0.0f, fb = n_ok ? p.fb[n] : 0.0f;
+  const float ws = (ASYM && n_ok) ? p.wsum[n] : 0.0f;
 
   // per-token epilogue operands, requested with the first activation fragments: their L2 round
   // trip is over long before the partial sums meet
@@ -265,6 +282,8 @@ cudaError_t launch_w4a4_decode(const GemmLaunch& g) {
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
   static_assert(kTileRows % (2 * kRows) == 0, "a CTA's row groups must not straddle two weight boxes");
   DecodeParams p{};
+  p.header = reinterpret_cast<const uint32_t*>(base);
+  p.status = g.status_word;
   p.tiles = base + h.off_tiles;
   p.sw = reinterpret_cast<const float*>(base + h.off_sw);
   p.fb = reinterpret_cast<const float*>(base + h.off_fb);

@@ -34,6 +34,8 @@
 // (|256 * acc| <= 256 * 64 * K < 2^31 for K <= 131072); acc = raw >> 8 is exact.
 #include <cuda.h>
 
+#include <mutex>
+
 #include "epilogue_math.cuh"
 #include "kernels.cuh"
 #include "ptx.cuh"
@@ -64,11 +66,12 @@ constexpr int kEpiWarp0 = 4;            // epilogue warps start here (warp % 4 =
 constexpr int kNumUnpackWarps = 4;      // per set
 constexpr int kAStageBytes = BM * BK;   // fused variant: int8 A operand stage in shared memory
 
-// CG = CTAs per tile (1 or 2).  FUSED = quantise-in-producer variant (a10): the eight A warps read
-// bf16 X, quantise with the per-token scale and write the int8 operand to SHARED memory (any
-// thread -> element mapping is allowed there; the Hadamard needs 16 lanes per 128 channels), and
-// the MMA takes both operands from shared memory (.ss form).
-template <int CG, bool FUSED>
+// A tile belongs to a CTA pair (cta_group::2, M = 256).  FUSED = quantise-in-producer variant
+// (a10): the eight A warps read bf16 X, quantise with the per-token scale and write the int8
+// operand to SHARED memory (any thread -> element mapping is allowed there; the Hadamard needs 16
+// lanes per 128 channels), and the MMA takes both operands from shared memory (.ss form).
+constexpr int CG = 2;                   // CTAs per tile
+template <bool FUSED>
 struct Cfg {
   // per-tile column operands of the epilogue (s_w, fb, wsum), one copy per accumulator stage
   static constexpr int kColParamBytes = kAccStages * 3 * BN * 4;
@@ -93,7 +96,7 @@ struct Cfg {
   static constexpr int kPEmptyCount = FUSED ? kNumUnpackWarps : kNumUnpackWarps + 4;
   static constexpr int kFullCount = CG * ((FUSED ? 8 : 4) + kNumUnpackWarps);
   static constexpr int kTemptyCount = CG * kEpiWarps;
-  static constexpr int kPStages = CG == 2 ? kPStagesMax : 5;
+  static constexpr int kPStages = kPStagesMax;
   static constexpr int kSmemBytes =
       1024 + kAOperand + kStages * kUnpackedStage + kPStages * kPackedStage + kTailBytes + kStoreBytes;
   static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
@@ -110,6 +113,8 @@ struct __align__(8) Barriers {
 static_assert(sizeof(Barriers) <= 256, "barrier block too large");
 
 struct GemmParams {
+  const uint32_t* header;   // blob header: magic, N, K, Npad, ... (checked against N, K below)
+  unsigned int* status;     // device status word: kStatusBadBlob is raised on a mismatch
   const uint8_t* tiles;     // blob boxes
   const float* sw;          // [Npad]
   const float* fb;          // [Npad]
@@ -211,14 +216,13 @@ __device__ __forceinline__ void dequant_bracket_asym(int32_t raw, float st256, f
 }
 
 // ------------------------------------------------------------------------------ the kernel
-// CG = 1: one CTA per tile of 128 x BN;  CG = 2: a CTA pair per tile of 256 x BN.
 // ASYM (NEXT-1): unsigned activation codes, re-centred to q - 8 while they are expanded, and the
 // epilogue term (z_t + 8 s_t) s_w wsum[n].
-template <int CG, bool FUSED, bool ASYM>
-__global__ void __launch_bounds__((Cfg<CG, FUSED>::kThreads), 1)
+template <bool FUSED, bool ASYM>
+__global__ void __launch_bounds__((Cfg<FUSED>::kThreads), 1)
 w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_y,
                  const GemmParams p) {
-  using C = Cfg<CG, FUSED>;
+  using C = Cfg<FUSED>;
   constexpr int kEpiWarps = C::kEpiWarps;
   constexpr int kSets = C::kSets;
   constexpr int kAWarp0 = C::kAWarp0;
@@ -239,8 +243,13 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
-  const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
+  const uint32_t rank = ptx::cluster_ctarank();
   const bool leader = rank == 0;
+  // The blob's header (written by the packer's first kernel, complete long before any dependent
+  // launch can start: see w4a4_decode.cu) is requested now and compared with the call's (N, K) after
+  // the prologue: a blob packed for another shape would be read out of bounds, so such a call does
+  // no work at all and raises the status word (baseq_sync_status -> BASEQ_ERR_WORKSPACE).
+  const uint4 hdr = ptx::ldg_nc(reinterpret_cast<const uint4*>(p.header));
 
   if (warp == kProducerWarp && lane == 0) {
     if (!FUSED) ptx::prefetch_tensormap(&tmap_a);
@@ -260,19 +269,21 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     ptx::fence_barrier_init();
   }
   if (warp == kMmaWarp) {
-    if (CG == 2) ptx::tmem_alloc_2cta<kTmemCols>(ptx::smem_u32(&bars->tmem_base));
-    else ptx::tmem_alloc<kTmemCols>(ptx::smem_u32(&bars->tmem_base));
+    ptx::tmem_alloc_2cta<kTmemCols>(ptx::smem_u32(&bars->tmem_base));
   }
   ptx::tcgen05_fence_before();
   __syncthreads();
-  if (CG == 2) ptx::cluster_sync_all();       // peer barriers initialised before any remote arrive
+  ptx::cluster_sync_all();                    // peer barriers initialised before any remote arrive
   ptx::tcgen05_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
   // prologue done (barriers, TMEM, tensor maps): from here on the predecessor's outputs are read
   ptx::griddep_launch_dependents();
   ptx::griddep_wait();
 
-  const int num_tiles = p.num_m * p.num_n;
+  const bool blob_ok = hdr.x == kBlobMagic && hdr.y == static_cast<uint32_t>(p.N) &&
+                       hdr.z == static_cast<uint32_t>(p.K);
+  if (!blob_ok && threadIdx.x == 0 && blockIdx.x == 0) atomicOr(p.status, kStatusBadBlob);
+  const int num_tiles = blob_ok ? p.num_m * p.num_n : 0;
   const int first_tile = static_cast<int>(blockIdx.x) / CG;
   const int tile_step = static_cast<int>(gridDim.x) / CG;
   const int n_it = first_tile < num_tiles
@@ -288,9 +299,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
       const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
       const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM;
-      // row groups of kTileRows rows: this CTA streams CG == 2 ? one : both of the tile's groups
-      const uint8_t* g0 = p.tiles + static_cast<size_t>(2 * n_blk + (CG == 2 ? rank : 0)) *
-                                        p.num_kb * kTileBytes;
+      // row groups of kTileRows rows: this CTA streams its half of the tile's N rows
+      const uint8_t* g0 = p.tiles + static_cast<size_t>(2 * n_blk + rank) * p.num_kb * kTileBytes;
       for (int kb = 0; kb < p.num_kb; ++kb) {
         ptx::mbar_wait(ptx::smem_u32(&bars->pempty[stage]), phase ^ 1u);
         const uint32_t full = ptx::smem_u32(&bars->pfull[stage]);
@@ -304,11 +314,6 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
             ptx::mbar_arrive_expect_tx(full, C::kPackedB);
             ptx::bulk_load_1d(dst + C::kPackedAArea, g0 + static_cast<size_t>(kb) * kTileBytes,
                               kTileBytes, full);
-            if (CG == 1) {
-              ptx::bulk_load_1d(dst + C::kPackedAArea + kTileBytes,
-                                g0 + static_cast<size_t>(p.num_kb + kb) * kTileBytes, kTileBytes,
-                                full);
-            }
           }
         }
         __syncwarp();
@@ -354,24 +359,20 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
                 const uint32_t accum = (k != 0 || kb != 0) ? 1u : 0u;
                 if (FUSED) {
                   const uint64_t da = adesc0 + static_cast<uint64_t>(stage * (kAStageBytes >> 4)) + 2 * k;
-                  if (CG == 2) ptx::mma_i8_ss_2cta(tmem_d, da, db + 2 * k, idesc, accum);
-                  else ptx::mma_i8_ss(tmem_d, da, db + 2 * k, idesc, accum);
+                  ptx::mma_i8_ss_2cta(tmem_d, da, db + 2 * k, idesc, accum);
                 } else {
-                  if (CG == 2) ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
-                  else ptx::mma_i8_ts(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
+                  ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
                 }
               }
               // frees the operand stage (A columns + B smem) in every CTA of the pair
-              if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
-              else ptx::tcgen05_commit(ptx::smem_u32(&bars->empty[stage]));
+              ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
             }
             __syncwarp();
             if (++kb == p.num_kb) {
               // tile complete: publish the accumulator, move to the other accumulator stage
               kb = 0;
               if (ptx::elect_one()) {
-                if (CG == 2) ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->tfull[as]), 3);
-                else ptx::tcgen05_commit(ptx::smem_u32(&bars->tfull[as]));
+                ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->tfull[as]), 3);
               }
               __syncwarp();
               advance(as, aphase, kAccStages);
@@ -730,11 +731,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     ptx::bulk_wait_group<0>();                          // Y stores complete before the CTA exits
   ptx::tcgen05_fence_before();
   __syncthreads();
-  if (CG == 2) ptx::cluster_sync_all();
+  ptx::cluster_sync_all();
   if (warp == kMmaWarp) {
     ptx::tcgen05_fence_after();
-    if (CG == 2) ptx::tmem_dealloc_2cta<kTmemCols>(tmem_base);
-    else ptx::tmem_dealloc<kTmemCols>(tmem_base);
+    ptx::tmem_dealloc_2cta<kTmemCols>(tmem_base);
   }
 }
 
@@ -751,31 +751,86 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 EncodeTiledFn get_encode_fn() {
   // resolved through the runtime so that libbaseq.so has no link-time dependency on libcuda
+  static std::once_flag once;
   static EncodeTiledFn fn = nullptr;
-  if (fn == nullptr) {
+  std::call_once(once, []() {
     void* sym = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) ==
             cudaSuccess && qres == cudaDriverEntryPointSuccess) {
       fn = reinterpret_cast<EncodeTiledFn>(sym);
     }
-  }
+  });
   return fn;
 }
 
-template <int CG, bool FUSED, bool ASYM>
-cudaError_t launch_cg(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, const GemmParams& p, int num_sms,
-                      cudaStream_t stream) {
-  using C = Cfg<CG, FUSED>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(w4a4_gemm_kernel<CG, FUSED, ASYM>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
+// 2-D row-major tensor map (SWIZZLE_64B boxes), memoised: a tensor map is a pure function of
+// (address, extents, row pitch, box, element type), and a serving loop calls the GEMM with the same
+// handful of buffers over and over -- the driver's encode call costs about as much as the rest of
+// the launch path.  Small direct-mapped table under a mutex (any host thread, any device: device
+// pointers of different GPUs are distinct in the unified address space).
+struct TmapKey {
+  const void* ptr;
+  uint64_t d0, d1, pitch;
+  uint32_t b0, b1, type, l2;
+  bool operator==(const TmapKey& o) const {
+    return ptr == o.ptr && d0 == o.d0 && d1 == o.d1 && pitch == o.pitch && b0 == o.b0 && b1 == o.b1 &&
+           type == o.type && l2 == o.l2;
   }
+};
+struct TmapSlot {
+  bool valid = false;
+  TmapKey key{};
+  CUtensorMap map{};
+};
+constexpr int kTmapSlots = 256;
+
+cudaError_t tensor_map_2d(const void* ptr, uint64_t d0, uint64_t d1, uint64_t pitch_bytes, uint32_t b0,
+                          uint32_t b1, CUtensorMapDataType type, CUtensorMapL2promotion l2,
+                          CUtensorMap* out) {
+  static std::mutex mu;
+  static TmapSlot table[kTmapSlots];
+  const TmapKey key{ptr, d0, d1, pitch_bytes, b0, b1, static_cast<uint32_t>(type), static_cast<uint32_t>(l2)};
+  uint64_t h = reinterpret_cast<uintptr_t>(ptr) * 0x9E3779B97F4A7C15ull;
+  h ^= (d0 * 0xC2B2AE3D27D4EB4Full) ^ (d1 * 0x165667B19E3779F9ull) ^ (pitch_bytes << 7) ^ (b1 << 3) ^ type;
+  TmapSlot& slot = table[(h >> 40) % kTmapSlots];
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    if (slot.valid && slot.key == key) {
+      *out = slot.map;
+      return cudaSuccess;
+    }
+  }
+  EncodeTiledFn encode = get_encode_fn();
+  if (encode == nullptr) return cudaErrorNotSupported;
+  const cuuint64_t dims[2] = {d0, d1};
+  const cuuint64_t strides[1] = {pitch_bytes};
+  const cuuint32_t box[2] = {b0, b1};
+  const cuuint32_t estr[2] = {1, 1};
+  CUtensorMap m{};
+  const CUresult r = encode(&m, type, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, l2,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    slot.valid = true;
+    slot.key = key;
+    slot.map = m;
+  }
+  *out = m;
+  return cudaSuccess;
+}
+
+template <bool FUSED, bool ASYM>
+cudaError_t launch_pair(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, const GemmParams& p,
+                        int num_sms, int device, cudaStream_t stream) {
+  using C = Cfg<FUSED>;
+  static std::atomic<int> attr_smem[kMaxDevices];
+  const cudaError_t ea = ensure_dynamic_smem(w4a4_gemm_kernel<FUSED, ASYM>, C::kSmemBytes, device, attr_smem);
+  if (ea != cudaSuccess) return ea;
   const int tiles = p.num_m * p.num_n;
-  const int slots = num_sms / CG;                        // CTAs (CG = 1) or CTA pairs (CG = 2)
+  const int slots = num_sms / CG;                        // CTA pairs
   const int groups = tiles < slots ? tiles : slots;
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(static_cast<unsigned>(groups * CG), 1, 1);
@@ -791,7 +846,7 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, cons
   attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 2;
-  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<CG, FUSED, ASYM>, tmap_a, tmap_y, p);
+  return cudaLaunchKernelEx(&cfg, w4a4_gemm_kernel<FUSED, ASYM>, tmap_a, tmap_y, p);
 }
 
 }  // namespace
@@ -799,44 +854,29 @@ cudaError_t launch_cg(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, cons
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   const bool fused = g.x != nullptr;
   if (!fused && g.T <= kDecodeMaxT) return launch_w4a4_decode(g);   // decode shapes: W-streaming kernel
-  if (fused && g.had_block > 128) return cudaErrorNotSupported;   // 16 lanes hold 128 channels
+  if (fused && (!fused_supported(g.had_block) || g.zeros != nullptr)) return cudaErrorNotSupported;
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
-  constexpr int cg = 2;   // CTA pairs; the kernel template keeps CG = 1 (one CTA per 128 x BN tile)
-                          // for reference, but it is not instantiated
 
   // A operand (unfused): codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows, SWIZZLE_64B;
   // rows beyond T are zero-filled by TMA, so a ragged last M tile needs no special case.
-  CUtensorMap tmap_a{};
-  if (!fused) {
-    EncodeTiledFn encode = get_encode_fn();
-    if (encode == nullptr) return cudaErrorNotSupported;
-    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(g.K / 2), static_cast<cuuint64_t>(g.T)};
-    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(g.K / 2)};
-    const cuuint32_t box[2] = {static_cast<cuuint32_t>(BK / 2), static_cast<cuuint32_t>(BM)};
-    const cuuint32_t estr[2] = {1, 1};
-    const CUresult r = encode(&tmap_a, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
-                              const_cast<uint8_t*>(g.codes), dims, strides, box, estr,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
-                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-  }
   // Y (unfused): bf16 [T, ldy]; box = 32 columns (64 bytes) x 32 rows, SWIZZLE_64B; the store clips
   // rows >= T and columns >= N.
-  CUtensorMap tmap_y{};
+  CUtensorMap tmap_a{}, tmap_y{};
   if (!fused) {
-    EncodeTiledFn encode = get_encode_fn();
-    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(g.N), static_cast<cuuint64_t>(g.T)};
-    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(g.ldy) * 2};
-    const cuuint32_t box[2] = {32, 32};
-    const cuuint32_t estr[2] = {1, 1};
-    const CUresult r = encode(&tmap_y, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, g.y, dims, strides, box, estr,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
-                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    cudaError_t e = tensor_map_2d(g.codes, static_cast<uint64_t>(g.K / 2), static_cast<uint64_t>(g.T),
+                                  static_cast<uint64_t>(g.K / 2), BK / 2, BM, CU_TENSOR_MAP_DATA_TYPE_UINT8,
+                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, &tmap_a);
+    if (e != cudaSuccess) return e;
+    e = tensor_map_2d(g.y, static_cast<uint64_t>(g.N), static_cast<uint64_t>(g.T),
+                      static_cast<uint64_t>(g.ldy) * 2, 32, 32, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+                      CU_TENSOR_MAP_L2_PROMOTION_NONE, &tmap_y);
+    if (e != cudaSuccess) return e;
   }
 
   GemmParams p{};
+  p.header = reinterpret_cast<const uint32_t*>(base);
+  p.status = g.status_word;
   p.tiles = base + h.off_tiles;
   p.sw = reinterpret_cast<const float*>(base + h.off_sw);
   p.fb = reinterpret_cast<const float*>(base + h.off_fb);
@@ -849,7 +889,7 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   p.T = g.T;
   p.N = g.N;
   p.K = g.K;
-  p.num_m = (g.T + BM * cg - 1) / (BM * cg);
+  p.num_m = (g.T + BM * CG - 1) / (BM * CG);
   p.num_n = h.Npad / BN;
   p.num_kb = g.K / BK;
   if (fused) {
@@ -861,11 +901,43 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
     p.had_block = g.had_block;
     p.had_scale = g.had_scale;
     p.codes_dump = reinterpret_cast<uint32_t*>(g.codes_dump);
-    if (g.zeros != nullptr) return cudaErrorNotSupported;   // fused + asymmetric: not built
-    return launch_cg<2, true, false>(tmap_a, tmap_y, p, g.num_sms, g.stream);
+    return launch_pair<true, false>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
   }
-  if (g.zeros != nullptr) return launch_cg<2, false, true>(tmap_a, tmap_y, p, g.num_sms, g.stream);
-  return launch_cg<2, false, false>(tmap_a, tmap_y, p, g.num_sms, g.stream);
+  if (g.zeros != nullptr) return launch_pair<false, true>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
+  return launch_pair<false, false>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
+}
+
+// ------------------------------------------------------------------------------ fused variant (a10)
+size_t fused_workspace_bytes(int T, int N, int K) {
+  (void)T; (void)N; (void)K;
+  return 256;   // the quantise-in-producer kernel keeps everything on chip
+}
+
+bool fused_supported(int had_block) { return had_block <= 128; }   // 16 lanes hold 128 channels
+
+cudaError_t launch_linear_fused(const GemmLaunch& g) {
+  // pass 1: per-token absmax -> scales (reads X once, writes T floats)
+  QuantLaunch q{};
+  q.x = g.x;
+  q.ldx = g.ldx;
+  q.T = g.T;
+  q.K = g.K;
+  q.alpha = g.alpha;
+  q.gamma = g.gamma;
+  q.sa = g.sa;
+  q.b = g.b;
+  q.had_block = g.had_block;
+  q.had_scale = g.had_scale;
+  q.codes = nullptr;
+  q.scales = const_cast<float*>(g.scales);
+  q.stream = g.stream;
+  q.num_sms = g.num_sms;
+  q.device = g.device;
+  q.blocks_per_sm = 2;
+  const cudaError_t e = launch_quantize_act(q, false);
+  if (e != cudaSuccess) return e;
+  // pass 2: GEMM with the quantise-in-producer warps
+  return launch_w4a4_gemm(g);
 }
 
 }  // namespace baseq

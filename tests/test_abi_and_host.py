@@ -38,7 +38,7 @@ def test_header_symbols_are_exported():
 
 def test_version_and_status_strings():
     _, L = _lib()
-    assert L.baseq_version() >= 1
+    assert L.baseq_version() >= 2
     seen = set()
     for code in range(8):
         s = L.baseq_status_string(code).decode()
@@ -84,6 +84,22 @@ def test_validation_happens_before_any_launch():
     f = L.baseq_linear_fused
     assert f(base, 256, 4, 256, ctypes.byref(ok), base, 8, base, 8, base, 0, None, base, None,
              None) == 5                                                            # workspace
+    # the fused and the host-buffer entry points run every check of BOTH stages before the first
+    # launch or copy (a failing call enqueues nothing): these all fail before the device is queried
+    had256 = P(0.9, 1.0, None, None, 256)
+    assert f(base, 256, 4, 256, ctypes.byref(had256), base, 8, base, 8, base, 4096, None, base, None,
+             None) == 6                                                            # fused: had_block > 128
+    bad_alpha = P(0.0, 1.0, None, None, 0)
+    assert f(base, 256, 4, 256, ctypes.byref(bad_alpha), base, 8, base, 8, base, 4096, None, base, None,
+             None) == 4
+    assert f(base, 256, 4, 256, ctypes.byref(ok), base, 12, base, 16, base, 4096, None, base, None,
+             None) == 2                                                            # N % 8 (second stage)
+    h = L.baseq_linear_host
+    assert h(base, 4, 256, ctypes.byref(bad_alpha), base, 8, base, base, 1 << 20, None) == 4
+    assert h(base, 4, 65536, ctypes.byref(ok), base, 8, base, base, 1 << 30, None) == 2
+    assert h(base, 4, 256, ctypes.byref(ok), base, 8, base, base, 16, None) == 5   # scratch too small
+    assert g(base, base, base, 4, 8, 65536, base, 8, None, None) == 2              # K <= 32768 everywhere
+    assert L.baseq_packed_weight_bytes(8, 65536) == 0
     assert L.baseq_pack_weights(base, base, None, None, 8, 128, base + 16, None, None) == 3
     kv = L.baseq_quantize_kv
     assert kv(None, 1024, 4, 8, 128, 1.0, base, base, base, None) == 1               # NULL

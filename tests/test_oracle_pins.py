@@ -408,6 +408,7 @@ def test_epilogue_against_exact_rational():
         for n in range(N):
             exact = Fraction(float(st[t])) * Fraction(float(sw[n])) * int(acc[t, n]) + Fraction(float(fb[n]))
             assert abs(Fraction(float(y64[t, n])) - exact) <= abs(exact) * Fraction(1, 2 ** 52)
+            assert y64[t, n] == float(exact)        # s_t s_w is exact in double: the fma is ONE rounding
             assert y[t, n] == _bf16_exact(float(y64[t, n]))
 
 
@@ -553,6 +554,37 @@ def test_asym_gemm_and_epilogue_identity():
                         + Fraction(float(z[t]))) for k in range(K)) + Fraction(float(fb[n]))
             assert Fraction(float(y64[t, n])) == exact          # powers of two: no rounding at all
             assert y[t, n] == oracle.bf16_from_double(float(exact))
+
+
+def test_asym_epilogue_against_exact_rational_on_general_scales():
+    # oracle_epilogue_asym on scales that are NOT powers of two (every fma really rounds):
+    #   c = fma(z s_w, wsum, fb);  y64 = fma(s s_w, acc, c)
+    # s s_w and z s_w are exact in double (24 x 24 bits), so each fma is ONE rounding of an exact
+    # rational; int / int true division in Python is correctly rounded, so float(Fraction) is that
+    # rounding.  Equality is required bit for bit, and the pin must tell the stated nesting from the
+    # other one (lower-bound term added last), which differs on some elements.
+    rng = np.random.default_rng(131)
+    T, N = 20, 36
+    acc = rng.integers(0, 900000, size=(T, N)).astype(np.int32)          # unsigned codes: acc >= 0 mostly
+    wsum = rng.integers(-30000, 30000, size=N).astype(np.int32)
+    st = (np.abs(rng.standard_normal(T)) * 0.3 + 0.013).astype(np.float32)
+    zt = (-8.3 * st * (1.0 + 0.2 * rng.standard_normal(T))).astype(np.float32)
+    sw = (np.abs(rng.standard_normal(N)) * 0.004 + 0.0011).astype(np.float32)
+    fb = rng.standard_normal(N).astype(np.float32)
+    y, y64 = oracle.epilogue_asym(acc, wsum, st, zt, sw, fb, return_y64=True)
+    other_nesting_differs = 0
+    for t in range(T):
+        for n in range(N):
+            S, Z, W, F = (Fraction(float(v)) for v in (st[t], zt[t], sw[n], fb[n]))
+            c = float(Z * W * int(wsum[n]) + F)                         # one rounding
+            want = float(S * W * int(acc[t, n]) + Fraction(c))          # one rounding
+            assert y64[t, n] == want, (t, n)
+            assert y[t, n] == _bf16_exact(want)
+            exact = S * W * int(acc[t, n]) + Z * W * int(wsum[n]) + F
+            assert abs(Fraction(want) - exact) <= (abs(Fraction(c)) + abs(exact)) * Fraction(1, 2 ** 52)
+            c2 = float(S * W * int(acc[t, n]) + F)
+            other_nesting_differs += float(Z * W * int(wsum[n]) + Fraction(c2)) != want
+    assert other_nesting_differs > 0
 
 
 # =========================================================================== NEXT-3: KV cache
