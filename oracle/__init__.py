@@ -19,4 +19,7 @@ from .binding import (  # noqa: F401
     epilogue_asym,
     linear_asym,
     quantize_kv,
+    dense_hadamard_u64,
+    dense_mode_bounds,
+    dense_mode_check,
 )

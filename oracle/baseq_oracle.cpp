@@ -372,6 +372,51 @@ int oracle_epilogue_asym(const int32_t* acc, const int32_t* wsum, const float* s
   return 0;
 }
 
-int oracle_version(void) { return 2; }
+// =======================================================================================
+// NEXT-2: the online Hadamard as a DENSE matrix product -- what the paper deploys
+// ("we avoid using it and instead implement it as a larger matrix multiplication"; R_qk as
+// a 128 x 128 matmul P:218) and what a tensor-core kernel computes.  A tensor core accumulates in
+// an unspecified order, so this mode has no bit-level contract: the oracle gives the EXACT values
+// (fp64; every product +-x is exact, the 128-term sums are exact unless the exponents of one block
+// spread over more than ~40 bits) and the tests accept a result iff it lies inside a stated band
+// around them.
+//   h[t, c]  = (1 / sqrt(B)) * sum_k H[c mod B][k] x[t, B (c div B) + k],  H[c][k] = (-1)^popcount(c & k)
+//              (Sylvester order: the same matrix the butterflies of oracle_hadamard_blocks apply,
+//              Eq. 2)
+//   u64[t,c] = g_c h[t,c] - b_c                       (Eq. 15), all in fp64
+//   l1[t, j] = sum_k |x[t, B j + k]|                  (the scale of block j's accumulation error)
+// Parity status: pinned (equals scipy.linalg.hadamard @ x in fp64; equals the butterfly oracle bit
+// for bit on integer inputs, where both are exact; H H = B I) -- tests/test_oracle_pins.py.
+// =======================================================================================
+int oracle_dense_hadamard_u64(const uint16_t* x_bf16, int64_t ldx, int T, int K, float gamma,
+                              const float* sa, const float* b, int B, double* u64, double* l1) {
+  if (T < 1 || K < 2 || B < 2 || (B & (B - 1)) != 0 || K % B != 0) return 2;
+  const double c = 1.0 / std::sqrt(static_cast<double>(B));
+  std::vector<double> x(static_cast<size_t>(B));
+  for (int t = 0; t < T; ++t) {
+    for (int j = 0; j < K / B; ++j) {
+      double a1 = 0.0;
+      for (int k = 0; k < B; ++k) {
+        x[k] = static_cast<double>(bf16_bits_to_float(x_bf16[static_cast<int64_t>(t) * ldx + j * B + k]));
+        a1 += std::fabs(x[k]);
+      }
+      if (l1) l1[static_cast<int64_t>(t) * (K / B) + j] = a1;
+      for (int ch = 0; ch < B; ++ch) {
+        double s = 0.0;
+        for (int k = 0; k < B; ++k) {
+          const int neg = __builtin_popcount(static_cast<unsigned>(ch & k)) & 1;
+          s += neg ? -x[k] : x[k];
+        }
+        const int col = j * B + ch;
+        const double g = sa ? static_cast<double>(sa[col]) : static_cast<double>(gamma);
+        const double bk = b ? static_cast<double>(b[col]) : 0.0;
+        u64[static_cast<int64_t>(t) * K + col] = g * (s * c) - bk;
+      }
+    }
+  }
+  return 0;
+}
+
+int oracle_version(void) { return 3; }
 
 }  // extern "C"

@@ -61,6 +61,9 @@ def _load():
         lib.oracle_epilogue_asym.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
                                              c.c_void_p, c.c_void_p, c.c_int, c.c_int, c.c_void_p,
                                              c.c_void_p]
+        lib.oracle_dense_hadamard_u64.restype = c.c_int
+        lib.oracle_dense_hadamard_u64.argtypes = [c.c_void_p, c.c_int64, c.c_int, c.c_int, c.c_float,
+                                                  c.c_void_p, c.c_void_p, c.c_int, c.c_void_p, c.c_void_p]
         _lib = lib
     return _lib
 
@@ -236,3 +239,61 @@ def linear_asym(x_bf16, w_nibbles, w_scale, fb, alpha, gamma=1.0, sa=None, b=Non
     y, y64 = epilogue_asym(acc, wsum, scales, zeros, w_scale, fb, return_y64=True)
     return {"codes": codes, "scales": scales, "zeros": zeros, "acc": acc, "wsum": wsum, "y": y,
             "y64": y64}
+
+
+# ------------------------------------------------------------------ NEXT-2: dense (tensor-core) Hadamard
+def dense_hadamard_u64(x_bf16, had_block, gamma=1.0, sa=None, b=None):
+    """Exact (fp64) u = g * (H_B x) / sqrt(B) - b per block of had_block channels, and the L1 norm of
+    every block of x (the scale of a tensor core's accumulation error).  Returns (u64 [T,K], l1 [T,K/B])."""
+    _chk(x_bf16, np.uint16, "x_bf16")
+    T, K = x_bf16.shape
+    _chk(sa, np.float32, "sa")
+    _chk(b, np.float32, "b")
+    u = np.empty((T, K), dtype=np.float64)
+    l1 = np.empty((T, K // had_block), dtype=np.float64)
+    rc = _load().oracle_dense_hadamard_u64(_ptr(x_bf16), K, T, K, gamma, _ptr(sa), _ptr(b), had_block,
+                                           _ptr(u), _ptr(l1))
+    if rc:
+        raise ValueError("oracle_dense_hadamard_u64: invalid arguments (status %d)" % rc)
+    return u, l1
+
+
+def dense_mode_bounds(u64, l1, alpha, had_block, sa=None, gamma=1.0, eps=2.0 ** -16):
+    """The acceptance band of the dense (tensor-core) Hadamard mode: a result u' is
+    admissible iff |u' - u64| <= tol with tol[t,c] = eps * |g_c| * l1[t, block(c)] / sqrt(B) +
+    2^-21 |u64| (accumulation error of block(c)'s 128-term sum, then two fp32 roundings).  Returns
+    (tol [T,K], m_lo [T], m_hi [T]): the band of the row absmax."""
+    T, K = u64.shape
+    g = np.abs(sa.astype(np.float64)) if sa is not None else np.full(K, abs(float(gamma)))
+    tol = eps * g[None, :] * np.repeat(l1, had_block, axis=1) / np.sqrt(float(had_block)) + 2.0 ** -21 * np.abs(u64)
+    a = np.abs(u64)
+    return tol, (a - tol).max(axis=1).clip(min=0.0), (a + tol).max(axis=1)
+
+
+def dense_mode_check(codes, scales, u64, tol, m_lo, m_hi, alpha):
+    """True iff (codes, scales) is an admissible output of the dense Hadamard mode: every scale is
+    max((alpha m) / 7, 1e-12) for some absmax m inside [m_lo, m_hi] (up to the two fp32 roundings of
+    Q4), and every code q satisfies clamp(rne(lo)) <= q <= clamp(rne(hi)) where [lo, hi] is the image
+    of [u64 - tol, u64 + tol] under multiplication by the RECIPROCAL OF THE RETURNED SCALE, rounded
+    as in Q5 (rounding is monotonic, so this says: some admissible u rounds to q).  Returns
+    (ok, n_bad_scales, n_bad_codes)."""
+    s = scales.astype(np.float64)
+    a = np.float64(np.float32(alpha))
+    floor = np.float64(np.float32(1e-12))
+    s_lo = np.maximum(a * m_lo / 7.0, floor) * (1 - 2.0 ** -22)
+    s_hi = np.maximum(a * m_hi / 7.0, floor) * (1 + 2.0 ** -22)
+    bad_s = (s < s_lo) | (s > s_hi)
+    inv = (np.float32(1.0) / scales.astype(np.float32)).astype(np.float64)[:, None]
+    lo = (u64 - tol) * inv
+    hi = (u64 + tol) * inv
+    lo -= np.abs(lo) * 2.0 ** -22
+    hi += np.abs(hi) * 2.0 ** -22
+    q_lo = np.clip(np.rint(lo), -8, 7)
+    q_hi = np.clip(np.rint(hi), -8, 7)
+    lo_n = (codes & 0xF).astype(np.int16)
+    hi_n = (codes >> 4).astype(np.int16)
+    q = np.empty(u64.shape, dtype=np.int16)
+    q[:, 0::2] = np.where(lo_n >= 8, lo_n - 16, lo_n)
+    q[:, 1::2] = np.where(hi_n >= 8, hi_n - 16, hi_n)
+    bad_q = (q < q_lo) | (q > q_hi)
+    return (not bad_s.any()) and (not bad_q.any()), int(bad_s.sum()), int(bad_q.sum())

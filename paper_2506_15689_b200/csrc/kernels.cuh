@@ -90,7 +90,6 @@ cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes);
 // long rows (K >= 4096): bulk-TMA ring variant of the same contract (quantize_ring.cu)
 bool quantize_ring_supported(int K);
 cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes);
-bool quantize_ring_supports_sa(int K, int had_block);
 
 // ------------------------------------------------------------------ weight packer
 // ------------------------------------------------------------------ KV-cache quantiser (NEXT-3)

@@ -185,13 +185,11 @@ cudaError_t launch_hw(const QuantLaunch& q, int V) {
 static_assert(512 * kMaxV * 8 >= kMaxK, "a row of kMaxK channels fits 512 threads x kMaxV vectors");
 
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes) {
-  // the asymmetric variant (NEXT-1) lives in the ring kernels only, scalar s^a
-  if (q.asym) return q.sa != nullptr ? cudaErrorNotSupported : launch_quantize_ring(q, write_codes);
-  // long rows with the scalar s^a (every benchmark shape): bulk-TMA ring kernel; a per-channel
-  // s^a vector takes the ring's split kernel at K = 4096 and the register-resident kernel below
-  // otherwise
-  if (quantize_ring_supported(q.K) && (q.sa == nullptr || quantize_ring_supports_sa(q.K, q.had_block)))
-    return launch_quantize_ring(q, write_codes);
+  // the asymmetric variant (NEXT-1) lives in the ring kernels only (any K)
+  if (q.asym) return launch_quantize_ring(q, write_codes);
+  // long rows (every benchmark shape): bulk-TMA ring kernels; short rows: the register-resident
+  // kernel below
+  if (quantize_ring_supported(q.K)) return launch_quantize_ring(q, write_codes);
   const int nvec = q.K / 8;
   // smallest power-of-two threads-per-row (>= 32) with at most 4 vectors per thread (the fp32 row
   // segment plus the prefetched next segment must leave room for two 256-thread blocks per SM);

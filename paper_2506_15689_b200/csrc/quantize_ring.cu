@@ -1,16 +1,22 @@
-// Activation quantiser for long rows (K >= 4096): the same arithmetic contract as
-// quantize_act.cu (quant_math.cuh), fed by a bulk-TMA ring.
+// Activation quantiser for long rows (K >= 4096, and every K of the asymmetric variant): the
+// arithmetic contract of quant_math.cuh (Q0-Q7), fed by a bulk-TMA ring.
 //
-// Why: the register-resident row kernel keeps only its own loads in flight (32-64 KB per SM) and
-// measured 2.5-3.0 TB/s (profiles/).  Here one producer lane streams whole token rows
-// (row-contiguous cp.async.bulk copies, completion on an mbarrier) into a ring of shared-memory
-// stages that fills whatever the 227 KB allow -- 150-200 KB of loads in flight per SM, no
-// registers involved -- and 16 consumer warps (512 threads = one row wide, thread r owns the
-// 16-byte vectors r, r + 512, ...) read each stage once from shared memory, conflict-free.
+// One producer lane streams whole token rows (row-contiguous cp.async.bulk copies, completion on an
+// mbarrier) into a ring of shared-memory stages that fills whatever the 227 KB allow -- 150-200 KB
+// of loads in flight per SM, no registers involved -- and 16 consumer warps read each stage once
+// from shared memory, conflict-free.
 //
-// Per stage of RL rows: pass 1 (u = g h - b, absmax) -> the stage is released to the producer ->
-// block reduction (partials in smem, one designated warp per row finishes the max and computes
-// s_t and 1 / s_t once) -> pass 2 from registers (round, clamp, pack, store).
+// Per stage: pass 1 (u = g h - b, absmax) -> the stage is released to the producer -> reduction
+// (partials in smem, one designated thread per row finishes the max and computes s_t and 1 / s_t
+// once) -> pass 2 from registers (round, clamp, pack, store).
+//
+// Instruction budget (r2): with the mixed-precision fma (FHFMA.BF16 consumes the bf16 activations in
+// place), three-input max (FMNMX3), fma-with-magic rounding and the saturating nibble pack the two
+// passes cost 4 issue slots per element (FHFMA, 1/2 FMNMX3, FFMA, IADD, 1/2 I2IP) instead of the ~9
+// of r1 (unpack, FFMA, FMNMX, FFMA, IADD, I2IP plus address arithmetic).
+#include <cstdlib>
+#include <cstring>
+
 #include "kernels.cuh"
 #include "ptx.cuh"
 #include "quant_math.cuh"
@@ -18,22 +24,32 @@
 namespace baseq {
 namespace {
 
-constexpr int kConsumers = 512;                 // threads per row
+constexpr int kConsumers = 512;                 // threads per row (row-wide kernel)
 constexpr int kConsumerWarps = kConsumers / 32;
 constexpr int kRingThreads = kConsumers + 32;   // + the producer warp
 constexpr int kMaxStages = 8;
 constexpr int kRingSmemBudget = 220 * 1024;
+constexpr float kNegHuge = -3.402823466e38f;
+
+// How the scale factor g of u = g h - b reaches the kernel:
+//   kGBf16  scalar s^a that is itself a bf16 value (1.0 in four of the five BASELINE configs): the
+//           mixed-precision fma consumes the bf16 activations in place (quant_math.cuh), no unpack
+//   kGF32   any other scalar s^a: unpack + FFMA
+//   kGVec   per-channel s^a vector (Eq. 15; NEXT-4): the thread's values live in private
+//           slots of shared memory behind the ring (V <= 4) or come through L1 for every row
+enum : int { kGBf16 = 0, kGF32 = 1, kGVec = 2 };
 
 struct RingParams {
   const uint8_t* x;        // bf16 rows
   int64_t row_bytes_stride;
   int T, K, nvec;
   float alpha, gamma;
+  uint32_t gamma_bf16;     // the scalar s^a as a bf16 bit pattern (kGBf16 only)
   const float* bvec;
-  const float* sa;         // per-channel s^a (split kernel only), or NULL for the scalar gamma
+  const float* sa;         // per-channel s^a (kGVec), else NULL
   int had_block;
   float had_scale;
-  uint32_t* codes;
+  uint32_t* codes;         // NULL: scales only (the fused GEMM's absmax pre-pass)
   float* scales;
   float* zeros;            // asymmetric variant only
   int stages;
@@ -60,7 +76,57 @@ cudaError_t launch_pdl(Kern kern, int blocks, int threads, int smem, cudaStream_
   return cudaLaunchKernelEx(&cfg, kern, p);
 }
 
-template <int V, int RL, bool HAD, bool WRITE_CODES, bool RAGGED, bool ASYM>
+// ------------------------------------------------------------------ shared pieces
+// The producer: one lane streams the RL rows of every stage this CTA owns.
+template <int RL>
+__device__ __forceinline__ void produce_rows(const RingParams& p, uint8_t* ring, uint64_t* full,
+                                             uint64_t* empty, int num_groups) {
+  int s = 0;
+  uint32_t ph = 0;
+  const uint32_t row_bytes = static_cast<uint32_t>(p.K) * 2u;
+  for (int g = blockIdx.x; g < num_groups; g += gridDim.x) {
+    ptx::mbar_wait(ptx::smem_u32(&empty[s]), ph ^ 1u);
+    const int row0 = g * RL;
+    const int rows = (p.T - row0) < RL ? (p.T - row0) : RL;
+    const uint32_t bar = ptx::smem_u32(&full[s]);
+    ptx::mbar_arrive_expect_tx(bar, row_bytes * rows);
+    const uint32_t dst = ptx::smem_u32(ring) + s * p.stage_bytes;
+    for (int j = 0; j < rows; ++j) {
+      ptx::bulk_load_1d(dst + j * row_bytes, p.x + static_cast<int64_t>(row0 + j) * p.row_bytes_stride,
+                        row_bytes, bar);
+    }
+    if (++s == p.stages) { s = 0; ph ^= 1u; }
+  }
+}
+
+// Q0-Q2 for one 16-byte vector: u = g h - b.  `g8` is read for kGVec only.
+template <bool HAD, int GMODE>
+__device__ __forceinline__ void vector_u(const RingParams& p, const uint4& xv, const float (&b8)[8],
+                                         const float (&g8)[8], int lane, float (&u)[8]) {
+  if (!HAD && GMODE == kGBf16) {
+    float nb[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) nb[e] = -b8[e];          // folds into the fma's operand modifier
+    qm::affine8_bf16(xv, p.gamma_bf16, nb, u);
+  } else {
+    float f[8];
+    qm::unpack8(xv, f);
+    if (HAD) qm::hadamard8(f, p.had_block, p.had_scale, lane);
+#pragma unroll
+    for (int e = 0; e < 8; ++e) u[e] = qm::affine(GMODE == kGVec ? g8[e] : p.gamma, f[e], b8[e]);
+  }
+}
+
+__device__ __forceinline__ void load8_shared(const float4* s, float (&v)[8]) {
+  const float4 a = s[0], b = s[1];
+  v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+  v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+}
+
+// ------------------------------------------------------------------ row-wide kernel
+// 512 threads = one row wide, thread r owns the 16-byte vectors r, r + 512, ... of all RL rows of a
+// stage, so its slice of b stays in registers for every row (V <= 4).
+template <int V, int RL, bool HAD, bool RAGGED, bool ASYM, int GMODE>
 __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const RingParams p) {
   extern __shared__ __align__(128) uint8_t ring[];
   __shared__ uint64_t full[kMaxStages], empty[kMaxStages];
@@ -85,41 +151,30 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
   ptx::griddep_wait();
 
   if (warp == kConsumerWarps) {
-    // ===================================================================== producer
-    if (lane == 0) {
-      int s = 0;
-      uint32_t ph = 0;
-      const uint32_t row_bytes = static_cast<uint32_t>(p.K) * 2u;
-      for (int g = blockIdx.x; g < num_groups; g += gridDim.x) {
-        ptx::mbar_wait(ptx::smem_u32(&empty[s]), ph ^ 1u);
-        const int row0 = g * RL;
-        const int rows = (p.T - row0) < RL ? (p.T - row0) : RL;
-        const uint32_t bar = ptx::smem_u32(&full[s]);
-        ptx::mbar_arrive_expect_tx(bar, row_bytes * rows);
-        const uint32_t dst = ptx::smem_u32(ring) + s * p.stage_bytes;
-        for (int j = 0; j < rows; ++j) {
-          ptx::bulk_load_1d(dst + j * row_bytes, p.x + static_cast<int64_t>(row0 + j) * p.row_bytes_stride,
-                            row_bytes, bar);
-        }
-        if (++s == p.stages) { s = 0; ph ^= 1u; }
-      }
-    }
+    if (lane == 0) produce_rows<RL>(p, ring, full, empty, num_groups);
     return;
   }
 
   // ======================================================================= consumers
   const int r = tid;                               // vector r + i * 512 of every row
-  constexpr bool kBiasInRegs = V <= 4;
-  float bb[kBiasInRegs ? V : 1][8];
-  if (kBiasInRegs) {
+  constexpr bool kInRegs = V <= 4;                 // b in registers, s^a in private smem slots
+  float bb[kInRegs ? V : 1][8];
+  float4* sa_s = reinterpret_cast<float4*>(ring + static_cast<size_t>(p.stages) * p.stage_bytes);
+  if (kInRegs) {
 #pragma unroll
     for (int i = 0; i < V; ++i) {
       const int idx = r + i * kConsumers;
-      if (p.bvec != nullptr && (!RAGGED || idx < p.nvec)) {
-        qm::load8_pinned(p.bvec + 8 * idx, bb[kBiasInRegs ? i : 0]);
+      const bool ok = !RAGGED || idx < p.nvec;
+      if (p.bvec != nullptr && ok) {
+        qm::load8_pinned(p.bvec + 8 * idx, bb[kInRegs ? i : 0]);
       } else {
 #pragma unroll
-        for (int e = 0; e < 8; ++e) bb[kBiasInRegs ? i : 0][e] = 0.0f;
+        for (int e = 0; e < 8; ++e) bb[kInRegs ? i : 0][e] = 0.0f;
+      }
+      if (GMODE == kGVec) {
+        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        sa_s[2 * idx] = ok ? __ldg(reinterpret_cast<const float4*>(p.sa) + 2 * idx) : z4;
+        sa_s[2 * idx + 1] = ok ? __ldg(reinterpret_cast<const float4*>(p.sa) + 2 * idx + 1) : z4;
       }
     }
   }
@@ -137,34 +192,30 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
     float m2[RL];                                      // asymmetric only: running max of -u
 #pragma unroll
     for (int j = 0; j < RL; ++j) {
-      m[j] = ASYM ? -3.402823466e38f : 0.0f;
-      m2[j] = -3.402823466e38f;
+      m[j] = ASYM ? kNegHuge : 0.0f;
+      m2[j] = kNegHuge;
+    }
 #pragma unroll
-      for (int i = 0; i < V; ++i) {
-        const int idx = r + i * kConsumers;
-        const bool ok = !RAGGED || idx < p.nvec;
+    for (int i = 0; i < V; ++i) {
+      const int idx = r + i * kConsumers;
+      const bool ok = !RAGGED || idx < p.nvec;
+      float b8[8], g8[8];
+      if (kInRegs) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) b8[e] = bb[kInRegs ? i : 0][e];
+        if (GMODE == kGVec) load8_shared(sa_s + 2 * idx, g8);
+      } else {
+        qm::load_gb(GMODE == kGVec ? p.sa : nullptr, p.bvec, p.gamma, idx, ok, g8, b8);
+      }
+#pragma unroll
+      for (int j = 0; j < RL; ++j) {
         uint4 xv = make_uint4(0, 0, 0, 0);
         if (ok) xv = *reinterpret_cast<const uint4*>(stage + static_cast<size_t>(j) * p.K * 2 + idx * 16);
-        float f[8];
-        qm::unpack8(xv, f);
-        if (HAD) qm::hadamard8(f, p.had_block, p.had_scale, lane);
-        float bl[8];
-        if (!kBiasInRegs) {
-          float g_unused[8];
-          qm::load_gb(nullptr, p.bvec, p.gamma, idx, ok, g_unused, bl);
-        }
-#pragma unroll
-        for (int e = 0; e < 8; ++e) {
-          const float bv = kBiasInRegs ? bb[kBiasInRegs ? i : 0][e] : bl[e];
-          u[j][i][e] = qm::affine(p.gamma, f[e], bv);          // scalar s^a only (see the launcher)
-          if (ASYM) {
-            if (ok) {
-              m[j] = fmaxf(m[j], u[j][i][e]);
-              m2[j] = fmaxf(m2[j], -u[j][i][e]);
-            }
-          } else {
-            m[j] = fmaxf(m[j], fabsf(u[j][i][e]));
-          }
+        vector_u<HAD, GMODE>(p, xv, b8, g8, lane, u[j][i]);
+        if (ASYM) {
+          if (ok) qm::maxmin8(m[j], m2[j], u[j][i]);
+        } else {
+          m[j] = qm::absmax8(m[j], u[j][i]);
         }
       }
     }
@@ -220,9 +271,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
     }
     named_barrier_sync(1, kConsumers);
     if (warp < RL) {
-      float mm = lane < kConsumerWarps ? s_part[parity][warp][lane] : (ASYM ? -3.402823466e38f : 0.0f);
-      float mm2 = (ASYM && lane < kConsumerWarps) ? s_part2[ASYM ? parity : 0][warp][lane]
-                                                  : -3.402823466e38f;
+      float mm = lane < kConsumerWarps ? s_part[parity][warp][lane] : (ASYM ? kNegHuge : 0.0f);
+      float mm2 = (ASYM && lane < kConsumerWarps) ? s_part2[ASYM ? parity : 0][warp][lane] : kNegHuge;
 #pragma unroll
       for (int o = 8; o > 0; o >>= 1) {
         mm = fmaxf(mm, __shfl_xor_sync(0xffffffffu, mm, o));
@@ -241,7 +291,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
     named_barrier_sync(2, kConsumers);
 
     // ---- pass 2: round, clamp, pack, store
-    if (WRITE_CODES) {
+    if (p.codes != nullptr) {
 #pragma unroll
       for (int j = 0; j < RL; ++j) {
         const float inv = s_scale[parity][j].y;
@@ -266,15 +316,18 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_kernel(const Ri
 // belongs to group j (thread r' of the group owns vectors r', r' + 128, ...).  Same work per
 // thread and stage as the row-wide layout (32 elements, one reduction, two barriers), but the
 // barriers are group-local, so while one group waits for its row's s_t (shuffles, barrier, two IEEE
-// divisions, barrier: ~1 us of latency in the row-wide kernel, where all 16 warps waited together)
-// the other three keep the issue slots busy.
-constexpr int kSplitGroups = 4;
-constexpr int kGroupThreads = kConsumers / kSplitGroups;   // 128
+// divisions, barrier) the other three keep the issue slots busy.
+constexpr int kGroupThreads = 128;
 constexpr int kGroupWarps = kGroupThreads / 32;
 
-template <int V, bool WRITE_CODES, bool ASYM, bool SA>
-__global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(const RingParams p) {
-  constexpr int RL = kSplitGroups;
+// G groups of 128 threads (+ the producer warp).  G = 4: one CTA per SM with the whole shared memory
+// as its ring.  G = 2: a CTA of 288 threads and half the shared memory, so that the NEXT kernel's CTA
+// is already resident (prologue done, parked in griddepcontrol.wait) while this one streams -- the
+// hand-over between two launches then costs one DRAM round trip instead of a CTA launch on top.
+template <int V, int G, bool ASYM, int GMODE>
+__global__ void __launch_bounds__(G * kGroupThreads + 32, G == 4 ? 1 : 2) quantize_ring_split_kernel(const RingParams p) {
+  constexpr int RL = G;
+  constexpr int kWarps = G * kGroupWarps;          // consumer warps
   extern __shared__ __align__(128) uint8_t ring[];
   __shared__ uint64_t full[kMaxStages], empty[kMaxStages];
   __shared__ float s_part[2][RL][kGroupWarps];
@@ -289,7 +342,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
   if (tid == 0) {
     for (int s = 0; s < p.stages; ++s) {
       ptx::mbar_init(ptx::smem_u32(&full[s]), 1);
-      ptx::mbar_init(ptx::smem_u32(&empty[s]), kConsumerWarps);
+      ptx::mbar_init(ptx::smem_u32(&empty[s]), kWarps);
     }
     ptx::fence_barrier_init();
   }
@@ -297,25 +350,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
   ptx::griddep_launch_dependents();
   ptx::griddep_wait();
 
-  if (warp == kConsumerWarps) {
-    if (lane == 0) {
-      int s = 0;
-      uint32_t ph = 0;
-      const uint32_t row_bytes = static_cast<uint32_t>(p.K) * 2u;
-      for (int g = blockIdx.x; g < num_groups; g += gridDim.x) {
-        ptx::mbar_wait(ptx::smem_u32(&empty[s]), ph ^ 1u);
-        const int row0 = g * RL;
-        const int rows = (p.T - row0) < RL ? (p.T - row0) : RL;
-        const uint32_t bar = ptx::smem_u32(&full[s]);
-        ptx::mbar_arrive_expect_tx(bar, row_bytes * rows);
-        const uint32_t dst = ptx::smem_u32(ring) + s * p.stage_bytes;
-        for (int j = 0; j < rows; ++j) {
-          ptx::bulk_load_1d(dst + j * row_bytes, p.x + static_cast<int64_t>(row0 + j) * p.row_bytes_stride,
-                            row_bytes, bar);
-        }
-        if (++s == p.stages) { s = 0; ph ^= 1u; }
-      }
-    }
+  if (warp == kWarps) {
+    if (lane == 0) produce_rows<RL>(p, ring, full, empty, num_groups);
     return;
   }
 
@@ -337,7 +373,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
   // spilled), so this thread's V x 8 values of s^a live in shared memory behind the ring, written
   // and read by this thread only (every group writes the same values: a benign duplicate)
   float4* sa_s = reinterpret_cast<float4*>(ring + static_cast<size_t>(p.stages) * p.stage_bytes);
-  if (SA) {
+  if (GMODE == kGVec) {
 #pragma unroll
     for (int i = 0; i < V; ++i) {
       const int idx = r + i * kGroupThreads;
@@ -355,30 +391,18 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
     const uint8_t* srow = ring + s * p.stage_bytes + static_cast<size_t>(grp) * p.K * 2;
 
     float u[V][8];
-    float m = ASYM ? -3.402823466e38f : 0.0f;
-    float m2 = -3.402823466e38f;                    // asymmetric only: running max of -u
+    float m = ASYM ? kNegHuge : 0.0f;
+    float m2 = kNegHuge;                            // asymmetric only: running max of -u
     if (row_ok) {                                   // rows past T were not loaded
 #pragma unroll
       for (int i = 0; i < V; ++i) {
-        const uint4 xv = *reinterpret_cast<const uint4*>(srow + (r + i * kGroupThreads) * 16);
-        float f[8];
-        qm::unpack8(xv, f);
-        float gv[8];
-        if (SA) {
-          const float4 g0 = sa_s[2 * (r + i * kGroupThreads)], g1 = sa_s[2 * (r + i * kGroupThreads) + 1];
-          gv[0] = g0.x; gv[1] = g0.y; gv[2] = g0.z; gv[3] = g0.w;
-          gv[4] = g1.x; gv[5] = g1.y; gv[6] = g1.z; gv[7] = g1.w;
-        }
-#pragma unroll
-        for (int e = 0; e < 8; ++e) {
-          u[i][e] = qm::affine(SA ? gv[e] : p.gamma, f[e], bb[i][e]);
-          if (ASYM) {
-            m = fmaxf(m, u[i][e]);
-            m2 = fmaxf(m2, -u[i][e]);
-          } else {
-            m = fmaxf(m, fabsf(u[i][e]));
-          }
-        }
+        const int idx = r + i * kGroupThreads;
+        const uint4 xv = *reinterpret_cast<const uint4*>(srow + idx * 16);
+        float g8[8];
+        if (GMODE == kGVec) load8_shared(sa_s + 2 * idx, g8);
+        vector_u<false, GMODE>(p, xv, bb[i], g8, lane, u[i]);
+        if (ASYM) qm::maxmin8(m, m2, u[i]);
+        else m = qm::absmax8(m, u[i]);
       }
     }
     __syncwarp();
@@ -400,7 +424,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
       float mm = s_part[parity][grp][0];
 #pragma unroll
       for (int w = 1; w < kGroupWarps; ++w) mm = fmaxf(mm, s_part[parity][grp][w]);
-      float mm2 = -3.402823466e38f;
+      float mm2 = kNegHuge;
       if (ASYM) {
 #pragma unroll
         for (int w = 0; w < kGroupWarps; ++w) mm2 = fmaxf(mm2, s_part2[ASYM ? parity : 0][grp][w]);
@@ -416,7 +440,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
     }
     named_barrier_sync(5 + grp, kGroupThreads);
 
-    if (WRITE_CODES) {
+    if (p.codes != nullptr) {
       const float inv = s_scale[parity][grp].y;
       uint32_t* crow = p.codes + static_cast<int64_t>(row) * p.nvec;
 #pragma unroll
@@ -428,8 +452,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) quantize_ring_split_kernel(co
   }
 }
 
-template <int V, bool WC, bool ASYM, bool SA>
-cudaError_t launch_ring_split(const QuantLaunch& q) {
+// ------------------------------------------------------------------ host side
+RingParams make_params(const QuantLaunch& q, bool write_codes) {
   RingParams p{};
   p.x = static_cast<const uint8_t*>(q.x);
   p.row_bytes_stride = q.ldx * 2;
@@ -438,84 +462,106 @@ cudaError_t launch_ring_split(const QuantLaunch& q) {
   p.nvec = q.K / 8;
   p.alpha = q.alpha;
   p.gamma = q.gamma;
+  uint32_t gbits;
+  static_assert(sizeof(gbits) == sizeof(q.gamma), "float bits");
+  std::memcpy(&gbits, &q.gamma, sizeof gbits);
+  p.gamma_bf16 = gbits >> 16;
   p.bvec = q.b;
   p.sa = q.sa;
-  p.codes = reinterpret_cast<uint32_t*>(q.codes);
+  p.had_block = q.had_block;
+  p.had_scale = q.had_scale;
+  p.codes = write_codes ? reinterpret_cast<uint32_t*>(q.codes) : nullptr;
   p.scales = q.scales;
   p.zeros = q.zeros;
-  p.stage_bytes = kSplitGroups * q.K * 2;
-  const int sa_bytes = SA ? q.K * 4 : 0;
+  return p;
+}
+
+int gmode_of(const QuantLaunch& q) {
+  if (q.sa != nullptr) return kGVec;
+  uint32_t gbits;
+  std::memcpy(&gbits, &q.gamma, sizeof gbits);
+  return ((gbits & 0xFFFFu) == 0u && q.had_block == 0) ? kGBf16 : kGF32;
+}
+
+template <int V, int G, bool ASYM, int GMODE>
+cudaError_t launch_ring_split_g(const QuantLaunch& q, bool write_codes) {
+  RingParams p = make_params(q, write_codes);
+  p.stage_bytes = G * q.K * 2;
+  const int sa_bytes = GMODE == kGVec ? q.K * 4 : 0;
+  const int budget = G == 4 ? kRingSmemBudget : 108 * 1024;
+  int stages = (budget - sa_bytes) / p.stage_bytes;
+  p.stages = stages > kMaxStages ? kMaxStages : stages;
+  if (p.stages < 2) return cudaErrorInvalidValue;
+  const int smem = p.stages * p.stage_bytes + sa_bytes;
+  static std::atomic<int> attr_smem[kMaxDevices];
+  const cudaError_t ea = ensure_dynamic_smem(quantize_ring_split_kernel<V, G, ASYM, GMODE>, smem, q.device, attr_smem);
+  if (ea != cudaSuccess) return ea;
+  const int groups = (q.T + G - 1) / G;
+  const int blocks = groups < q.num_sms ? groups : q.num_sms;
+  return launch_pdl(quantize_ring_split_kernel<V, G, ASYM, GMODE>, blocks, G * kGroupThreads + 32, smem, q.stream, p);
+}
+
+template <int V, bool ASYM, int GMODE>
+cudaError_t launch_ring_split(const QuantLaunch& q, bool write_codes) {
+  static const int g_exp = getenv("BASEQ_SPLIT_G") ? atoi(getenv("BASEQ_SPLIT_G")) : 4;
+  return g_exp == 2 ? launch_ring_split_g<V, 2, ASYM, GMODE>(q, write_codes)
+                    : launch_ring_split_g<V, 4, ASYM, GMODE>(q, write_codes);
+}
+
+template <int V, int RL, bool HAD, bool RAGGED, bool ASYM, int GMODE>
+cudaError_t launch_ring_g(const QuantLaunch& q, bool write_codes) {
+  RingParams p = make_params(q, write_codes);
+  p.stage_bytes = RL * q.K * 2;
+  const int slots = (q.K / 8 + kConsumers - 1) / kConsumers * kConsumers;     // padded to whole threads
+  const int sa_bytes = (GMODE == kGVec && V <= 4) ? slots * 32 : 0;
   int stages = (kRingSmemBudget - sa_bytes) / p.stage_bytes;
   p.stages = stages > kMaxStages ? kMaxStages : stages;
   if (p.stages < 2) return cudaErrorInvalidValue;
   const int smem = p.stages * p.stage_bytes + sa_bytes;
   static std::atomic<int> attr_smem[kMaxDevices];
-  const cudaError_t ea = ensure_dynamic_smem(quantize_ring_split_kernel<V, WC, ASYM, SA>, smem, q.device, attr_smem);
-  if (ea != cudaSuccess) return ea;
-  const int groups = (q.T + kSplitGroups - 1) / kSplitGroups;
-  const int blocks = groups < q.num_sms ? groups : q.num_sms;
-  return launch_pdl(quantize_ring_split_kernel<V, WC, ASYM, SA>, blocks, kRingThreads, smem, q.stream, p);
-}
-
-template <int V, int RL, bool HAD, bool WC, bool RAGGED, bool ASYM>
-cudaError_t launch_ring_a(const QuantLaunch& q) {
-  RingParams p{};
-  p.x = static_cast<const uint8_t*>(q.x);
-  p.row_bytes_stride = q.ldx * 2;
-  p.T = q.T;
-  p.K = q.K;
-  p.nvec = q.K / 8;
-  p.alpha = q.alpha;
-  p.gamma = q.gamma;
-  p.bvec = q.b;
-  p.had_block = q.had_block;
-  p.had_scale = q.had_scale;
-  p.codes = reinterpret_cast<uint32_t*>(q.codes);
-  p.scales = q.scales;
-  p.zeros = q.zeros;
-  p.stage_bytes = RL * q.K * 2;
-  int stages = kRingSmemBudget / p.stage_bytes;
-  p.stages = stages > kMaxStages ? kMaxStages : stages;
-  if (p.stages < 2) return cudaErrorInvalidValue;
-  const int smem = p.stages * p.stage_bytes;
-  static std::atomic<int> attr_smem[kMaxDevices];
-  const cudaError_t ea = ensure_dynamic_smem(quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM>, smem, q.device, attr_smem);
+  const cudaError_t ea =
+      ensure_dynamic_smem(quantize_ring_kernel<V, RL, HAD, RAGGED, ASYM, GMODE>, smem, q.device, attr_smem);
   if (ea != cudaSuccess) return ea;
   const int groups = (q.T + RL - 1) / RL;
   const int blocks = groups < q.num_sms ? groups : q.num_sms;
-  return launch_pdl(quantize_ring_kernel<V, RL, HAD, WC, RAGGED, ASYM>, blocks, kRingThreads, smem, q.stream, p);
+  return launch_pdl(quantize_ring_kernel<V, RL, HAD, RAGGED, ASYM, GMODE>, blocks, kRingThreads, smem, q.stream, p);
 }
 
-template <int V, int RL, bool HAD, bool WC, bool RAGGED>
-cudaError_t launch_ring_r(const QuantLaunch& q) {
-  // the asymmetric variant (NEXT-1) always writes codes
-  if (q.asym) return WC ? launch_ring_a<V, RL, HAD, true, RAGGED, true>(q) : cudaErrorInvalidValue;
-  return launch_ring_a<V, RL, HAD, WC, RAGGED, false>(q);
+template <int V, int RL, bool HAD, bool RAGGED, bool ASYM>
+cudaError_t launch_ring_a(const QuantLaunch& q, bool wc, int gmode) {
+  if (gmode == kGVec) return launch_ring_g<V, RL, HAD, RAGGED, ASYM, kGVec>(q, wc);
+  if (gmode == kGBf16 && !HAD) return launch_ring_g<V, RL, HAD, RAGGED, ASYM, HAD ? kGF32 : kGBf16>(q, wc);
+  return launch_ring_g<V, RL, HAD, RAGGED, ASYM, kGF32>(q, wc);
 }
 
-template <int V, int RL, bool HAD, bool WC>
-cudaError_t launch_ring_t(const QuantLaunch& q) {
-  return (q.K / 8) % kConsumers != 0 ? launch_ring_r<V, RL, HAD, WC, true>(q)
-                                     : launch_ring_r<V, RL, HAD, WC, false>(q);
+template <int V, int RL, bool HAD>
+cudaError_t launch_ring_t(const QuantLaunch& q, bool wc, int gmode) {
+  const bool ragged = (q.K / 8) % kConsumers != 0;
+  if (q.asym) {
+    return ragged ? launch_ring_a<V, RL, HAD, true, true>(q, wc, gmode)
+                  : launch_ring_a<V, RL, HAD, false, true>(q, wc, gmode);
+  }
+  return ragged ? launch_ring_a<V, RL, HAD, true, false>(q, wc, gmode)
+                : launch_ring_a<V, RL, HAD, false, false>(q, wc, gmode);
 }
 
-template <bool HAD, bool WC>
-cudaError_t launch_ring_hw(const QuantLaunch& q, int V, int RL) {
+template <bool HAD>
+cudaError_t launch_ring_hw(const QuantLaunch& q, bool wc, int gmode, int V, int RL) {
   // reachable (V, RL): RL = 4 for K <= 5120 (V <= 2), RL = 2 for K <= 10240 (V = 2, 3), else RL = 1
   if (RL == 4) {
-    if (V == 1) return launch_ring_t<1, 4, HAD, WC>(q);
-    if (V == 2) return launch_ring_t<2, 4, HAD, WC>(q);
+    if (V == 1) return launch_ring_t<1, 4, HAD>(q, wc, gmode);
+    if (V == 2) return launch_ring_t<2, 4, HAD>(q, wc, gmode);
   } else if (RL == 2) {
-    if (V == 2) return launch_ring_t<2, 2, HAD, WC>(q);
-    if (V == 3) return launch_ring_t<3, 2, HAD, WC>(q);
+    if (V == 2) return launch_ring_t<2, 2, HAD>(q, wc, gmode);
+    if (V == 3) return launch_ring_t<3, 2, HAD>(q, wc, gmode);
   } else {
     switch (V) {
-      case 3: return launch_ring_t<3, 1, HAD, WC>(q);
-      case 4: return launch_ring_t<4, 1, HAD, WC>(q);
-      case 5: return launch_ring_t<5, 1, HAD, WC>(q);
-      case 6: return launch_ring_t<6, 1, HAD, WC>(q);
-      case 7: return launch_ring_t<7, 1, HAD, WC>(q);
-      case 8: return launch_ring_t<8, 1, HAD, WC>(q);
+      case 3: return launch_ring_t<3, 1, HAD>(q, wc, gmode);
+      case 4: return launch_ring_t<4, 1, HAD>(q, wc, gmode);
+      case 5: return launch_ring_t<5, 1, HAD>(q, wc, gmode);
+      case 6: return launch_ring_t<6, 1, HAD>(q, wc, gmode);
+      case 7: return launch_ring_t<7, 1, HAD>(q, wc, gmode);
+      case 8: return launch_ring_t<8, 1, HAD>(q, wc, gmode);
       default: break;
     }
   }
@@ -524,28 +570,26 @@ cudaError_t launch_ring_hw(const QuantLaunch& q, int V, int RL) {
 
 }  // namespace
 
-bool quantize_ring_supported(int K) { return K >= 4096 && K <= 32768; }
-// a per-channel s^a vector is handled by the split kernel only
-bool quantize_ring_supports_sa(int K, int had_block) { return K == 4096 && had_block == 0; }
+bool quantize_ring_supported(int K) { return K >= 4096 && K <= kMaxK; }
 
 cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes) {
+  if (q.asym && !write_codes) return cudaErrorInvalidValue;
   const int nvec = q.K / 8;
   const int V = (nvec + kConsumers - 1) / kConsumers;
   const int RL = q.K <= 5120 ? 4 : (q.K <= 10240 ? 2 : 1);
+  const int gmode = gmode_of(q);
   if (q.had_block == 0 && q.K == 4096) {
     if (q.asym) {
-      if (q.sa != nullptr || !write_codes) return cudaErrorInvalidValue;
-      return launch_ring_split<4, true, true, false>(q);
+      if (gmode == kGVec) return launch_ring_split<4, true, kGVec>(q, write_codes);
+      return gmode == kGBf16 ? launch_ring_split<4, true, kGBf16>(q, write_codes)
+                             : launch_ring_split<4, true, kGF32>(q, write_codes);
     }
-    if (q.sa != nullptr) {
-      return write_codes ? launch_ring_split<4, true, false, true>(q) : launch_ring_split<4, false, false, true>(q);
-    }
-    return write_codes ? launch_ring_split<4, true, false, false>(q) : launch_ring_split<4, false, false, false>(q);
+    if (gmode == kGVec) return launch_ring_split<4, false, kGVec>(q, write_codes);
+    return gmode == kGBf16 ? launch_ring_split<4, false, kGBf16>(q, write_codes)
+                           : launch_ring_split<4, false, kGF32>(q, write_codes);
   }
-  if (q.had_block) {
-    return write_codes ? launch_ring_hw<true, true>(q, V, RL) : launch_ring_hw<true, false>(q, V, RL);
-  }
-  return write_codes ? launch_ring_hw<false, true>(q, V, RL) : launch_ring_hw<false, false>(q, V, RL);
+  return q.had_block ? launch_ring_hw<true>(q, write_codes, gmode, V, RL)
+                     : launch_ring_hw<false>(q, write_codes, gmode, V, RL);
 }
 
 }  // namespace baseq

@@ -95,7 +95,7 @@ def test_quantizer_per_channel_sa_long_rows():
     # a per-channel s^a vector: the ring's split kernel at K = 4096 without Hadamard, the
     # register-resident kernel otherwise
     rng = np.random.default_rng(17)
-    for K in (4096, 11008):
+    for K in (4096, 8192, 11008, 14336, 28672):
         x = rand_x(rng, 9, K)
         b = (0.5 * rng.standard_normal(K)).astype(np.float32)
         sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
@@ -603,14 +603,15 @@ def test_random_shapes_and_parameters():
 
 
 # ------------------------------------------------------------------------------- NEXT-1: asymmetric
-def run_asym(x_bits, W, alpha, gamma, b, had_block=0, rows=None):
+def run_asym(x_bits, W, alpha, gamma, b, had_block=0, rows=None, sa=None):
     """baseq_quantize_act_asym + baseq_w4a4_gemm_asym vs the oracle, everything bit for bit."""
     N, K = W["N"], W["K"]
     T = x_bits.shape[0]
     fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
     pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None if b is None else dev(b),
                          None if W["layer_bias"] is None else dev(W["layer_bias"]))
-    params = bq.ActParams(alpha, gamma, None, None if b is None else dev(b), had_block)
+    params = bq.ActParams(alpha, gamma, None if sa is None else dev(sa), None if b is None else dev(b),
+                          had_block)
     codes, scales, zeros = bq.quantize_act_asym(bf16_dev(x_bits), params)
     acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
     y = bq.w4a4_gemm_asym(codes, scales, zeros, pw, acc_dump=acc)
@@ -619,7 +620,7 @@ def run_asym(x_bits, W, alpha, gamma, b, had_block=0, rows=None):
     assert torch.equal(y.view(torch.int16), y2.view(torch.int16))
     sel = np.arange(T) if rows is None else rows
     ref = oracle.linear_asym(np.ascontiguousarray(x_bits[sel]), W["w_nibbles"], W["w_scale"], fb,
-                             alpha, gamma, None, b, had_block)
+                             alpha, gamma, sa, b, had_block)
     assert np.array_equal(scales.cpu().numpy()[sel].view(np.uint32), ref["scales"].view(np.uint32))
     assert np.array_equal(zeros.cpu().numpy()[sel].view(np.uint32), ref["zeros"].view(np.uint32))
     assert np.array_equal(codes.cpu().numpy()[sel], ref["codes"])
@@ -660,12 +661,16 @@ def test_asym_degenerate_rows_and_offsets():
     run_asym(f32_to_bf16_bits(x), W, 0.5, 1.0, None)
 
 
-def test_asym_rejects_per_channel_sa():
-    x = torch.zeros((4, 256), dtype=torch.bfloat16, device="cuda")
-    sa = torch.ones(256, device="cuda")
-    with pytest.raises(bq.BaseqError) as e:
-        bq.quantize_act_asym(x, bq.ActParams(0.9, 1.0, sa))
-    assert e.value.status == 6
+@pytest.mark.parametrize("T,K,N,B", [(9, 256, 72, 0), (70, 4096, 136, 0), (33, 11008, 72, 0),
+                                     (12, 14336, 64, 128), (5, 28672, 64, 128)])
+def test_asym_per_channel_sa(T, K, N, B):
+    # NEXT-4 second half: the per-channel s^a vector (Eq. 15) through the asymmetric
+    # quantiser (the paper's deployed setting), every ring-kernel instantiation family
+    rng = np.random.default_rng(17 * T + K + N + B)
+    x = rand_x(rng, T, K, spread=1.0)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+    run_asym(x, _rand_w(rng, N, K), 0.9, 1.0, b, had_block=B, sa=sa)
 
 
 # =========================================================================== NEXT-3: KV cache

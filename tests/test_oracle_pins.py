@@ -656,3 +656,77 @@ def test_rounding_is_of_the_exact_product():
             alpha = np.nextafter(alpha, f32(2.0))
     assert found["below"] > 0 and found["above"] > 0     # the search exercised both sides
     assert separating > 0
+
+
+# =========================================================================== NEXT-2: dense Hadamard mode
+def test_dense_hadamard_equals_library_matrix_product():
+    # oracle_dense_hadamard_u64 against scipy.linalg.hadamard (Sylvester construction, the library
+    # routine) applied in fp64: u = g * (H x) / sqrt(B) - b, per block
+    from scipy.linalg import hadamard
+    rng = np.random.default_rng(61)
+    for B, K in ((128, 384), (16, 64), (2, 8)):
+        x = bf16(rng.standard_normal((5, K)) * 3.0)
+        xf = bf16_bits_to_f32(x).astype(np.float64)
+        sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+        b = rng.standard_normal(K).astype(np.float32)
+        u, l1 = oracle.dense_hadamard_u64(x, B, 1.0, sa, b)
+        H = hadamard(B).astype(np.float64)
+        want = (xf.reshape(5, K // B, B) @ H.T).reshape(5, K) / np.sqrt(B) * sa.astype(np.float64) - b
+        assert np.allclose(u, want, rtol=0, atol=1e-12 * np.abs(want).max())
+        assert np.allclose(l1, np.abs(xf).reshape(5, K // B, B).sum(axis=2), rtol=1e-15)
+
+
+def test_dense_hadamard_equals_butterflies_where_both_are_exact():
+    # small-integer inputs: every butterfly of Q1 is exact in fp32 and the dense sum is exact in
+    # fp64, so the two oracle modes must agree (before the 1/sqrt(B) rounding: use B = 4, 16, 64,
+    # whose 1/sqrt(B) is a power of two)
+    rng = np.random.default_rng(62)
+    for B in (4, 16, 64):
+        K = 4 * B
+        xi = rng.integers(-60, 61, size=(3, K)).astype(np.float32)
+        x = bf16(xi)
+        u, _ = oracle.dense_hadamard_u64(x, B)
+        for t in range(3):
+            h = bf16_bits_to_f32(x[t]).copy()
+            oracle.hadamard_blocks(h, B)
+            assert np.array_equal(h.astype(np.float64), u[t])
+    # and H H = B I: applying the dense transform twice returns the input (g = 1, b = 0, exact here)
+    x = bf16(rng.integers(-7, 8, size=(2, 64)).astype(np.float32))
+    u, _ = oracle.dense_hadamard_u64(x, 16)
+    u2, _ = oracle.dense_hadamard_u64(bf16(u.astype(np.float32)), 16)
+    assert np.array_equal(u2, bf16_bits_to_f32(x).astype(np.float64))
+
+
+def test_dense_mode_band_accepts_the_contract_and_rejects_mistakes():
+    # The acceptance band of the tensor-core mode (oracle.dense_mode_check): the bit-exact
+    # butterfly quantiser is itself an admissible dense-mode result (its fp32 error is far inside the
+    # band); a result with a wrong sign convention, a dropped bias, or codes off by one level on
+    # elements that are not near a rounding boundary is rejected.
+    rng = np.random.default_rng(63)
+    T, K, B = 6, 1024, 128
+    x = bf16(rng.standard_normal((T, K)) + 0.3)
+    b = (0.3 * rng.standard_normal(K)).astype(np.float32)
+    u, l1 = oracle.dense_hadamard_u64(x, B, 1.0, None, b)
+    tol, m_lo, m_hi = oracle.dense_mode_bounds(u, l1, 0.9, B)
+    codes, scales = oracle.quantize_act(x, 0.9, 1.0, None, b, B)
+    ok, bs, bq_ = oracle.dense_mode_check(codes, scales, u, tol, m_lo, m_hi, 0.9)
+    assert ok, (bs, bq_)
+    # no bias
+    c2, s2 = oracle.quantize_act(x, 0.9, 1.0, None, None, B)
+    assert not oracle.dense_mode_check(c2, s2, u, tol, m_lo, m_hi, 0.9)[0]
+    # scale off by 2^-12
+    assert not oracle.dense_mode_check(codes, (scales * np.float32(1 + 2.0 ** -12)).astype(np.float32),
+                                       u, tol, m_lo, m_hi, 0.9)[0]
+    # one code moved by one level (an element in the middle of its rounding interval)
+    q = codes_to_int(codes)
+    r = u / scales[:, None].astype(np.float64)
+    t, k = np.unravel_index(np.argmin(np.abs(r - np.rint(r)) + 10.0 * (np.abs(q) >= 7)), r.shape)
+    q2 = q.copy()
+    q2[t, k] += 1
+    u8 = (q2.astype(np.int16) & 0xF).astype(np.uint8)
+    c3 = (u8[:, 0::2] | (u8[:, 1::2] << 4)).astype(np.uint8)
+    ok3, _, nb = oracle.dense_mode_check(c3, scales, u, tol, m_lo, m_hi, 0.9)
+    assert not ok3 and nb == 1
+    # the band is narrow: at most a small fraction of the elements may take two values
+    lo = np.rint((u - tol) / scales[:, None]); hi = np.rint((u + tol) / scales[:, None])
+    assert (lo != hi).mean() < 2e-3
