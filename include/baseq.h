@@ -121,6 +121,23 @@ BASEQ_API baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int
                                   const baseq_act_params_t* p, uint8_t* codes, float* scales,
                                   void* stream);
 
+/* ---- NEXT-2: the same quantiser with the online block-128 Hadamard run on the tensor cores --
+ * what the paper deploys ("implement it as a larger matrix multiplication"; R_qk as a
+ * 128 x 128 matmul): H_128 X^T with tcgen05.mma kind::f16, fp32 accumulation in tensor
+ * memory.  +-1 and the bf16 activations are exact operands; only the ORDER of each 128-term fp32
+ * sum is the tensor core's, so codes and scales are not bit-reproducible against
+ * baseq_quantize_act's fp32-butterfly contract.  Guarantee: with
+ *   u*[t,c] = g_c (H x)[t,c] / sqrt(128) - b_c      evaluated exactly,
+ *   tol[t,c] = 2^-16 |g_c| sum_{k in block(c)} |x[t,k]| / sqrt(128) + 2^-21 |u*[t,c]|,
+ * the returned s_t is max((alpha m) / 7, 1e-12) for an m inside the band of max_c |u*| +- tol, and
+ * every returned code is clamp(rne(u' / s_t), -8, 7) for some u' with |u' - u*| <= tol: a code can
+ * differ from the contract's only where u* / s_t is within tol / s_t of a rounding boundary, and then
+ * by one level.  Same arguments, layouts and errors as baseq_quantize_act; p->had_block must be 128
+ * and K <= 28672, else BASEQ_ERR_UNSUPPORTED.  The codes feed baseq_w4a4_gemm unchanged. */
+BASEQ_API baseq_status_t baseq_quantize_act_tc(const void* x_bf16, int64_t ldx, int T, int K,
+                                     const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                     void* stream);
+
 /* ---- W4A4 GEMM + fused de-quantisation (K1 + K3 of SURVEY) ----
  *   acc[t,n] = sum_k qa[t,k] * qw[n,k]                       exact int32 (tcgen05 kind::i8)
  *   Y[t,n]   = bf16_rne( (s_t * s_w[n]) * acc[t,n] + fb[n] ) evaluated as the fp64 expression

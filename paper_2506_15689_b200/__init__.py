@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     pack_weights,
     quantize_act,
     quantize_act_asym,
+    quantize_act_tc,
     w4a4_gemm_asym,
     quantize_kv,
     sync_status,

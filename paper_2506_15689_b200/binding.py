@@ -13,7 +13,7 @@ _lib = None
 
 EXPORTED_SYMBOLS = [
     "baseq_status_string", "baseq_version", "baseq_sync_status", "baseq_packed_weight_bytes", "baseq_pack_weights",
-    "baseq_set_fused_bias", "baseq_quantize_act", "baseq_w4a4_gemm",
+    "baseq_set_fused_bias", "baseq_quantize_act", "baseq_quantize_act_tc", "baseq_w4a4_gemm",
     "baseq_fused_workspace_bytes", "baseq_linear_fused", "baseq_linear_host_scratch_bytes",
     "baseq_linear_host", "baseq_quantize_act_asym", "baseq_w4a4_gemm_asym", "baseq_quantize_kv",
 ]
@@ -59,6 +59,8 @@ def lib():
         L.baseq_set_fused_bias.argtypes = [vp, i32, i32, vp, vp]
         L.baseq_quantize_act.restype = i32
         L.baseq_quantize_act.argtypes = [vp, i64, i32, i32, c.POINTER(_ActParamsC), vp, vp, vp]
+        L.baseq_quantize_act_tc.restype = i32
+        L.baseq_quantize_act_tc.argtypes = [vp, i64, i32, i32, c.POINTER(_ActParamsC), vp, vp, vp]
         L.baseq_w4a4_gemm.restype = i32
         L.baseq_w4a4_gemm.argtypes = [vp, vp, vp, i32, i32, i32, vp, i64, vp, vp]
         L.baseq_fused_workspace_bytes.restype = sz
@@ -153,6 +155,20 @@ def quantize_act(x, params, codes=None, scales=None):
     cs = params.c_struct()
     _check(lib().baseq_quantize_act(_p(x), x.stride(0), T, K, ctypes.byref(cs), _p(codes),
                                     _p(scales), _stream()), "baseq_quantize_act")
+    return codes, scales
+
+
+def quantize_act_tc(x, params, codes=None, scales=None):
+    """NEXT-2: quantize_act with the block-128 Hadamard on the tensor cores (tolerance parity)."""
+    T, K = x.shape
+    assert x.dtype == torch.bfloat16 and x.stride(1) == 1
+    if codes is None:
+        codes = torch.empty((T, K // 2), dtype=torch.uint8, device=x.device)
+    if scales is None:
+        scales = torch.empty((T,), dtype=torch.float32, device=x.device)
+    cs = params.c_struct()
+    _check(lib().baseq_quantize_act_tc(_p(x), x.stride(0), T, K, ctypes.byref(cs), _p(codes),
+                                       _p(scales), _stream()), "baseq_quantize_act_tc")
     return codes, scales
 
 

@@ -245,6 +245,21 @@ baseq_status_t baseq_quantize_act(const void* x_bf16, int64_t ldx, int T, int K,
   return from_cuda(launch_quantize_act(q, true));
 }
 
+baseq_status_t baseq_quantize_act_tc(const void* x_bf16, int64_t ldx, int T, int K,
+                                     const baseq_act_params_t* p, uint8_t* codes, float* scales,
+                                     void* stream) {
+  baseq_status_t st = validate_quant(x_bf16, ldx, T, K, p, codes, scales, true);
+  if (st != BASEQ_OK) return st;
+  if (!quantize_tc_supported(K, p->had_block)) return BASEQ_ERR_UNSUPPORTED;
+  DeviceRef d;
+  st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
+  q.num_sms = d.num_sms;
+  q.device = d.device;
+  return from_cuda(launch_quantize_tc(q));
+}
+
 baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scales, const void* packed_w,
                                int T, int N, int K, void* y_bf16, int64_t ldy, int32_t* acc_dump,
                                void* stream) {

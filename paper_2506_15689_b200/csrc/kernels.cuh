@@ -91,7 +91,10 @@ cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes);
 bool quantize_ring_supported(int K);
 cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes);
 
-// ------------------------------------------------------------------ weight packer
+// NEXT-2: the block-128 Hadamard on the tensor cores (quantize_had_tc.cu); tolerance parity
+bool quantize_tc_supported(int K, int had_block);
+cudaError_t launch_quantize_tc(const QuantLaunch& q);
+
 // ------------------------------------------------------------------ KV-cache quantiser (NEXT-3)
 struct KvLaunch {
   const void* x;        // bf16 [T, ldx], row t = heads blocks of head_dim channels

@@ -119,6 +119,101 @@ def test_quantizer_strided_input():
     assert np.array_equal(scales.cpu().numpy(), os_)
 
 
+# ------------------------------------------------------------------------------- NEXT-2: tensor-core Hadamard
+def check_quant_tc(x_bits, alpha, gamma=1.0, sa=None, b=None, rows=None):
+    """baseq_quantize_act_tc against the dense-Hadamard oracle mode: every scale and every code
+    must be admissible (oracle.dense_mode_check); beside it, the fraction of codes
+    that differ from the bit-exact butterfly contract (must be tiny: only elements whose u / s_t sits
+    within the band of a rounding boundary may move, and then by one level)."""
+    params = bq.ActParams(alpha, gamma, None if sa is None else dev(sa), None if b is None else dev(b), 128)
+    codes, scales = bq.quantize_act_tc(bf16_dev(x_bits), params)
+    torch.cuda.synchronize()
+    codes, scales = codes.cpu().numpy(), scales.cpu().numpy()
+    sel = np.arange(x_bits.shape[0]) if rows is None else rows
+    xs = np.ascontiguousarray(x_bits[sel])
+    u64, l1 = oracle.dense_hadamard_u64(xs, 128, gamma, sa, b)
+    tol, m_lo, m_hi = oracle.dense_mode_bounds(u64, l1, alpha, 128, sa, gamma)
+    ok, bad_s, bad_q = oracle.dense_mode_check(codes[sel], scales[sel], u64, tol, m_lo, m_hi, alpha)
+    assert ok, "tensor-core Hadamard: %d inadmissible scales, %d inadmissible codes" % (bad_s, bad_q)
+    ocodes, oscales = oracle.quantize_act(xs, alpha, gamma, sa, b, 128)
+    frac = float((codes[sel] != ocodes).mean())
+    assert frac < 2e-3, "too many codes differ from the butterfly contract: %.2e of the bytes" % frac
+    assert np.allclose(scales[sel], oscales, rtol=2.0 ** -18, atol=0)
+    return frac
+
+
+@pytest.mark.parametrize("T,K", [(16, 128), (1, 256), (37, 384), (100, 4096), (33, 11008), (21, 14336),
+                                 (50, 28672), (130, 3584), (17, 7168)])
+def test_quantizer_tc_shapes(T, K):
+    # one CTA (K <= 3584), clusters of 2 / 4 / 8 (uneven block split at K = 11008), ragged token groups
+    rng = np.random.default_rng(T * 7 + K)
+    x = rand_x(rng, T, K, 0.3)
+    b = (0.2 * rng.standard_normal(K)).astype(np.float32)
+    check_quant_tc(x, 0.9, 1.0, None, b)
+
+
+def test_quantizer_tc_variants():
+    rng = np.random.default_rng(909)
+    T, K = 45, 4096
+    x = rand_x(rng, T, K, 0.5)
+    b = (0.3 * rng.standard_normal(K)).astype(np.float32)
+    sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+    check_quant_tc(x, 1.0)                                # no bias, no clipping
+    check_quant_tc(x, 0.5, 1.2, None, b)                  # heavy clipping
+    check_quant_tc(x, 0.9, 1.0, sa, b)                    # per-channel s^a
+    zero = np.zeros((20, 256), dtype=np.uint16)           # floor scale, codes 0
+    params = bq.ActParams(0.9, 1.0, None, None, 128)
+    codes, scales = bq.quantize_act_tc(bf16_dev(zero), params)
+    torch.cuda.synchronize()
+    assert torch.all(codes == 0) and torch.all(scales == float(np.float32(1e-12)))
+    # small integers: the 128-term sums are exact in any order -- the transform itself must then be
+    # exact (one-hot rows spread a / sqrt(128) with the signs of H's columns, Eq. 2 P:59-64)
+    onehot = np.zeros((128, 128), dtype=np.float32)
+    onehot[np.arange(128), np.arange(128)] = 16.0
+    codes, scales = bq.quantize_act_tc(bf16_dev(f32_to_bf16_bits(onehot)), bq.ActParams(1.0, 1.0, None, None, 128))
+    torch.cuda.synchronize()
+    oc, os_ = oracle.quantize_act(f32_to_bf16_bits(onehot), 1.0, 1.0, None, None, 128)
+    assert np.array_equal(codes.cpu().numpy(), oc) and np.array_equal(scales.cpu().numpy(), os_)
+
+
+def test_quantizer_tc_config5_full_size_sampled_rows():
+    # config 5's activation at full size (T = 4096, K = 28672: clusters of 8, 16 groups per cluster)
+    L = cached_layer("c5", "down")
+    rows = half_rows(L["spec"].T)
+    frac = check_quant_tc(L["x"], L["spec"].alpha, L["spec"].gamma, None, L["b"], rows=rows)
+    assert frac < 1e-3
+
+
+def test_quantizer_tc_feeds_the_gemm():
+    # the codes of the tensor-core mode through the unchanged GEMM: the accumulators equal the
+    # oracle's integer GEMM of THOSE codes, the output its epilogue with THOSE scales
+    rng = np.random.default_rng(4711)
+    T, K, N = 130, 1024, 264
+    x = rand_x(rng, T, K, 0.3)
+    b = (0.2 * rng.standard_normal(K)).astype(np.float32)
+    W = _rand_w(rng, N, K)
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(b), dev(W["layer_bias"]))
+    codes, scales = bq.quantize_act_tc(bf16_dev(x), bq.ActParams(0.9, 1.0, None, dev(b), 128))
+    acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
+    y = bq.w4a4_gemm(codes, scales, pw, acc_dump=acc)
+    bq.sync_status()
+    oacc = oracle.gemm_i32(codes.cpu().numpy(), W["w_nibbles"])
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    assert np.array_equal(acc.cpu().numpy(), oacc)
+    assert np.array_equal(bits_host(y), oracle.epilogue(oacc, scales.cpu().numpy(), W["w_scale"], fb))
+
+
+def test_quantizer_tc_rejects_other_blocks():
+    x = torch.zeros((4, 256), dtype=torch.bfloat16, device="cuda")
+    for B in (0, 64, 256):
+        with pytest.raises(bq.BaseqError) as e:
+            bq.quantize_act_tc(x, bq.ActParams(0.9, had_block=B))
+        assert e.value.status == 6
+    with pytest.raises(bq.BaseqError) as e:
+        bq.quantize_act_tc(torch.zeros((4, 32768), dtype=torch.bfloat16, device="cuda"), bq.ActParams(0.9, had_block=128))
+    assert e.value.status == 6
+
+
 # ------------------------------------------------------------------------------- packer
 def test_pack_weights_fused_bias_matches_oracle():
     W = make_weights("c1", "linear")
