@@ -15,11 +15,13 @@
 //   A = H_128 (M = 128 output channels x K = 128 input channels, +-1 as bf16) lives in TENSOR MEMORY
 //       for the whole kernel (64 columns) -- no shared-memory traffic for it at all;
 //   B = tiles of X: 8 tokens x 128 channels per block, K-major, SWIZZLE_128B, streamed by TMA (one
-//       4-D tensor copy brings 8 blocks x 8 tokens = 16 KB laid out [half][block][token][64 ch]).
-//       H is the same matrix for every block, so the 8 x 8 (block, token) rows of a stage are the 64
-//       rows of ONE operand: one N = 64 instruction per K = 16 step serves eight blocks (an N = 16
-//       instruction costs ~35 clk, an N = 64 one ~75: cta_group::1 runs at half the tensor rate and
-//       every instruction re-reads the 4 KB of A).  Every element of X is read from HBM ONCE;
+//       4-D tensor copy brings up to 14 blocks x 8 tokens = 28 KB laid out [half][block][token][64 ch]).
+//       H is the same matrix for every block, so the (block, token) rows of a stage are the rows of
+//       ONE operand: one N = 112 instruction per K = 16 step serves fourteen blocks.  Measured
+//       (a probe of back-to-back instructions): an M = 128 kind::f16 MMA with A in tensor memory
+//       takes 130 clk whatever N is (16 ... 224) -- the 4 KB of A are re-read by every instruction
+//       at 32 B/clk -- so N must be as large as the data in flight allows (N = 16: 224 instructions
+//       and 29 k clk per 8 token rows; N = 112: 16 and 2.1 k).  Every element of X is read ONCE;
 //   D = 128 lanes (channels) x 8 columns (tokens) per block.  The CTA's share of a group of 8 token
 //       rows (<= 28 blocks = 3584 channels = 224 columns) stays RESIDENT in tensor memory while
 //       the epilogue warps read it twice -- pass 1 (u = g h - b written back over h, absmax), pass 2
@@ -29,6 +31,8 @@
 //   distributed shared memory (st.async + a transaction mbarrier).  A dedicated warp does the
 //   exchange and the two divisions while the epilogue warps are already in pass 1 of the NEXT group:
 //   no epilogue warp ever waits for another one (all hand-overs are mbarriers).
+//   The 16 epilogue warps form two teams of 8; a team owns one of the group's two slots (half of the
+//   CTA's blocks), so its waits concern that slot's MMAs only.
 //   Epilogue thread <-> data: tcgen05.ld.16x256b hands a thread two TMEM lanes (r, r + 8) and four
 //   columns; H's rows are permuted so that these two lanes are the channels 2j and 2j + 1 -- the two
 //   nibbles of one output byte -- so the saturating pack (cvt.pack.sat.s4.s32) builds whole bytes
@@ -49,13 +53,13 @@ namespace {
 
 constexpr int kTok = 8;                  // tokens per group
 constexpr int kBlk = 128;                // Hadamard block = MMA M = MMA K extent
-constexpr int kSB = 8;                   // blocks per TMA stage / per D slot (MMA N = 64)
+constexpr int kSBMax = 14;               // blocks per TMA stage / per D slot (MMA N <= 112); a group = 2 slots
+constexpr int kUPSMax = kSBMax / 2;      // epilogue units (two blocks each) of a warp: it owns ONE slot
 constexpr int kMaxBlocks = 28;           // per CTA: 28 x 8 = 224 D columns per group
-constexpr int kSlots = (kMaxBlocks + kSB - 1) / kSB;    // 4 (the last one half full)
 constexpr int kHCols = 64;               // A operand: 128 bf16 per lane
 constexpr int kDCols = kMaxBlocks * kTok;               // 224 columns per resident group
-constexpr int kXStages = 7;              // smem ring
-constexpr int kStageBytes = kSB * 2 * kTok * 128;       // [2 halves][8 blocks][8 tokens][128 B] = 16 KB
+constexpr int kXStages = 5;              // smem ring: 2.5 groups in flight
+constexpr int kStageBytes = kSBMax * 2 * kTok * 128;    // [2 halves][<= 14 blocks][8 tokens][128 B] = 28 KB
 constexpr int kCodePitch = kMaxBlocks * 64 + 16;        // bytes per token row of the codes tile (+16: banks)
 constexpr int kCodeTile = kTok * kCodePitch;
 constexpr int kMaxCluster = 8;
@@ -67,7 +71,7 @@ constexpr int kTcThreads = 640;
 
 struct TcBarriers {
   uint64_t xfull[kXStages], xempty[kXStages];
-  uint64_t dfull[2][kSlots], dempty[2][kSlots];   // a slot of a group's D buffer: MMAs done / pass 2 has it in registers (16 warps)
+  uint64_t dfull[2][2], dempty[2][2];    // [D buffer][slot]: MMAs done / pass 2 has the slot in registers (8 warps)
   uint64_t pmfull[2];                    // the 16 warps' partial maxima of a group are in wmax
   uint64_t xchg[4];                      // the cluster's partial maxima have arrived (transaction count)
   uint64_t invfull[2];                   // 1 / s_t of a group is in inv
@@ -76,8 +80,7 @@ struct TcBarriers {
 };
 
 struct TcSmem {                          // after the 1024-aligned X ring and the codes tiles
-  float gs[kMaxBlocks * kBlk];           // g_c / sqrt(128) of the CTA's channels
-  float bs[kMaxBlocks * kBlk];           // b_c
+  float4 gb[kMaxBlocks * kBlk / 2];      // per channel pair (2j, 2j + 1): g / sqrt(128) of both, then b of both
   float xmax[4][kMaxCluster][kTok];      // partial row maxima of every CTA of the cluster (see the scale warp)
   float wmax[2][kEpiWarps][kTok];
   float inv[2][kTok];
@@ -162,6 +165,9 @@ __device__ __forceinline__ void bulk_store_1d(void* gdst, uint32_t src_smem, uin
                : "memory");
 }
 
+// UPS = sb / 2: units (two blocks each) of an epilogue warp, a compile-time constant so that its
+// loops over tensor-memory loads unroll (a run-time trip count cost 2x on config 5)
+template <int UPS>
 __global__ void __launch_bounds__(kTcThreads, 1)
 quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -178,7 +184,9 @@ quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParam
   const int per = (p.nblk_total + static_cast<int>(csize) - 1) / static_cast<int>(csize);
   const int blk0 = static_cast<int>(rank) * per;
   const int nb = max(0, min(per, p.nblk_total - blk0));
-  const int nslots = (nb + kSB - 1) / kSB;
+  constexpr int sb = 2 * UPS;
+  const int nslots = (nb + sb - 1) / sb;                 // 0, 1 or 2
+  const uint32_t stage_bytes = static_cast<uint32_t>(sb) * 2u * kTok * 128u;
   const int num_groups = (p.T + kTok - 1) / kTok;
   // this cluster's groups: cluster_id, cluster_id + n_clusters, ...
   const int my_groups = cluster_id < num_groups ? (num_groups - cluster_id + n_clusters - 1) / n_clusters : 0;
@@ -190,9 +198,9 @@ quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParam
       ptx::mbar_init(ptx::smem_u32(&bars->xempty[i]), 1);
     }
     for (int i = 0; i < 2; ++i) {
-      for (int j = 0; j < kSlots; ++j) {
+      for (int j = 0; j < 2; ++j) {
         ptx::mbar_init(ptx::smem_u32(&bars->dfull[i][j]), 1);
-        ptx::mbar_init(ptx::smem_u32(&bars->dempty[i][j]), kEpiWarps);
+        ptx::mbar_init(ptx::smem_u32(&bars->dempty[i][j]), kEpiWarps / 2);
       }
       ptx::mbar_init(ptx::smem_u32(&bars->pmfull[i]), kEpiWarps);
       ptx::mbar_init(ptx::smem_u32(&bars->invfull[i]), 1);
@@ -231,11 +239,11 @@ quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParam
     ptx::tmem_st_wait();
   }
   // per-channel operands of the CTA's slice (parameters of the call, not a predecessor's output)
-  for (int i = threadIdx.x; i < nb * kBlk; i += kTcThreads) {
-    const int col = blk0 * kBlk + i;
-    const float g = p.sa != nullptr ? __ldg(p.sa + col) : p.gamma;
-    sm->gs[i] = __fmul_rn(g, p.had_scale);
-    sm->bs[i] = p.bvec != nullptr ? __ldg(p.bvec + col) : 0.0f;
+  for (int i = threadIdx.x; i < nb * kBlk / 2; i += kTcThreads) {
+    const int col = blk0 * kBlk + 2 * i;
+    const float g0 = p.sa != nullptr ? __ldg(p.sa + col) : p.gamma, g1 = p.sa != nullptr ? __ldg(p.sa + col + 1) : p.gamma;
+    sm->gb[i] = make_float4(__fmul_rn(g0, p.had_scale), __fmul_rn(g1, p.had_scale),
+                            p.bvec != nullptr ? __ldg(p.bvec + col) : 0.0f, p.bvec != nullptr ? __ldg(p.bvec + col + 1) : 0.0f);
   }
   ptx::tcgen05_fence_before();
   __syncthreads();
@@ -254,10 +262,10 @@ quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParam
         for (int j = 0; j < nslots; ++j) {
           ptx::mbar_wait(ptx::smem_u32(&bars->xempty[xs]), ph ^ 1u);
           const uint32_t bar = ptx::smem_u32(&bars->xfull[xs]);
-          ptx::mbar_arrive_expect_tx(bar, kStageBytes);
-          // box (64 channels, 8 tokens, 8 blocks, 2 halves of a block): rows >= T and blocks >= K / 128
+          ptx::mbar_arrive_expect_tx(bar, stage_bytes);
+          // box (64 channels, 8 tokens, sb blocks, 2 halves of a block): rows >= T and blocks >= K / 128
           // are zero-filled; blocks of a neighbouring CTA (last, partial slot) are read and ignored
-          tma_load_4d(ring0 + xs * kStageBytes, &tmap_x, 0, g * kTok, blk0 + j * kSB, 0, bar);
+          tma_load_4d(ring0 + xs * kStageBytes, &tmap_x, 0, g * kTok, blk0 + j * sb, 0, bar);
           if (++xs == kXStages) { xs = 0; ph ^= 1u; }
         }
       }
@@ -277,14 +285,14 @@ quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParam
           if (ptx::elect_one()) {
             // MMA N: the slot's blocks x 8 tokens, rounded up to the multiple of 16 that M = 128 needs
             // (an odd last block computes 8 spare columns that stay inside this group's D buffer)
-            const int blocks = min(kSB, nb - j * kSB);
+            const int blocks = min(sb, nb - j * sb);
             const uint32_t idesc = make_idesc_bf16(kBlk, static_cast<uint32_t>(((blocks * kTok + 15) / 16) * 16));
             const uint64_t desc0 = ptx::make_smem_desc_sw128(ring0 + xs * kStageBytes);
-            const uint32_t d = tmem_base + kHCols + buf * kDCols + static_cast<uint32_t>(j * kSB * kTok);
+            const uint32_t d = tmem_base + kHCols + buf * kDCols + static_cast<uint32_t>(j * sb * kTok);
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-              // half k / 4 of the block (8 KB further on), 32 bytes per K = 16 step inside the 128-byte row
-              const uint64_t db = desc0 + static_cast<uint64_t>(((k >> 2) * (kSB * kTok * 128) + (k & 3) * 32) >> 4);
+              // half k / 4 of the blocks (sb KB further on), 32 bytes per K = 16 step inside the 128-byte row
+              const uint64_t db = desc0 + static_cast<uint64_t>(((k >> 2) * (sb * kTok * 128) + (k & 3) * 32) >> 4);
               mma_f16_ts(d, tmem_base + 8 * k, db, idesc, k != 0 ? 1u : 0u);
             }
             ptx::tcgen05_commit(ptx::smem_u32(&bars->xempty[xs]));
@@ -354,74 +362,68 @@ quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParam
     }
   } else if (warp < kEpiWarps) {
     // ===================================================================== epilogue (16 warps)
-    // warp e: TMEM lane quarter e & 3 (fixed by the hardware), 16-lane half (e >> 2) & 1, and the
-    // blocks 4 (e >> 3) .. 4 (e >> 3) + 3 of every slot (two loads of two blocks each)
+    // warp e: TMEM lane quarter e & 3 (fixed by the hardware), 16-lane half (e >> 2) & 1, team e >> 3:
+    // the team owns slot `team` of every group (blocks team * sb ...), two blocks per load
     const int e = warp;
-    const int q = e & 3, hh = (e >> 2) & 1, bl0 = 4 * (e >> 3);
+    const int q = e & 3, hh = (e >> 2) & 1, team = e >> 3;
     const int lane_base = 32 * q + 16 * hh;              // this warp's 16 TMEM lanes
     const int r = lane >> 2, c = lane & 3;
-    const int ch_even = lane_base + 2 * r;               // channel (in the block) of TMEM lane lane_base + r
-    const int jbyte = lane_base / 2 + r;                 // byte column (in the block) of the channel pair
+    const int pair = lane_base / 2 + r;                  // channel pair (2 pair, 2 pair + 1) of the block =
+                                                         // TMEM lanes lane_base + r, + 8 = byte column
     const uint32_t taddr0 = tmem_base + (static_cast<uint32_t>(lane_base) << 16) + kHCols;
     // A load covers two blocks (lb, lb + 1) x this thread's tokens 2c, 2c + 1 x its two channels:
     // registers 0, 1 = (even channel, token 2c / 2c+1, block lb), 2, 3 = odd channel, 4..7 = block lb + 1.
-    // Units of a group: (slot j, pair i) -> blocks j * 8 + bl0 + 2 i, + 1; 2 per slot.
-    const int nunits = 2 * nslots;
-    auto unit_block = [&](int u) { return (u >> 1) * kSB + bl0 + 2 * (u & 1); };
+    const int bl0 = team * sb;
+    const int my_blocks = max(0, min(sb, nb - bl0));     // blocks of this team's slot
+    const int nunits = (my_blocks + 1) / 2;              // <= UPS
 
     // ---- pass 1 of group gi: u = g h - b written back over h, partial absmax of tokens 2c, 2c + 1
     auto pass1 = [&](int gi) {
       const uint32_t buf = static_cast<uint32_t>(gi) & 1u, phase = (static_cast<uint32_t>(gi) >> 1) & 1u;
-      const uint32_t tbuf = taddr0 + buf * kDCols;
+      const uint32_t tbuf = taddr0 + buf * kDCols + static_cast<uint32_t>(bl0 * kTok);
       float m0 = 0.0f, m1 = 0.0f;
-      uint32_t va[8], vb[8];
-      float2 ga[2], ba[2], gb[2], bb[2];
-      auto load = [&](int u, uint32_t (&v)[8], float2 (&gg)[2], float2 (&bv)[2]) {
-        if ((u & 1) == 0) {                                     // first unit of a slot: its MMAs are complete
-          ptx::mbar_wait(ptx::smem_u32(&bars->dfull[buf][u >> 1]), phase);
-          ptx::tcgen05_fence_after();
-        }
-        const int lb = min(unit_block(u), kMaxBlocks - 2);      // blocks >= nb: spare columns, results unused
-        tmem_ld_16x256b_x2(tbuf + static_cast<uint32_t>(lb * kTok), v);
+      if (nunits > 0) {
+        ptx::mbar_wait(ptx::smem_u32(&bars->dfull[buf][team]), phase);       // this slot's MMAs are complete
+        ptx::tcgen05_fence_after();
+        uint32_t va[8], vb[8];
+        float4 ga[2], gb[2];
+        auto load = [&](int u, uint32_t (&v)[8], float4 (&gg)[2]) {
+          tmem_ld_16x256b_x2(tbuf + static_cast<uint32_t>(2 * u * kTok), v);
 #pragma unroll
-        for (int i = 0; i < 2; ++i) {
-          gg[i] = *reinterpret_cast<const float2*>(&sm->gs[(lb + i) * kBlk + ch_even]);
-          bv[i] = *reinterpret_cast<const float2*>(&sm->bs[(lb + i) * kBlk + ch_even]);
-        }
-      };
-      auto math = [&](int u, const uint32_t (&v)[8], const float2 (&gg)[2], const float2 (&bv)[2]) {
-        const int lb = unit_block(u);
-        if (lb < nb) {
+          for (int i = 0; i < 2; ++i) gg[i] = sm->gb[min(bl0 + 2 * u + i, kMaxBlocks - 1) * (kBlk / 2) + pair];
+        };
+        auto math = [&](int u, const uint32_t (&v)[8], const float4 (&gg)[2]) {
           float uu[8];
-          uu[0] = qm::affine(gg[0].x, __uint_as_float(v[0]), bv[0].x);
-          uu[1] = qm::affine(gg[0].x, __uint_as_float(v[1]), bv[0].x);
-          uu[2] = qm::affine(gg[0].y, __uint_as_float(v[2]), bv[0].y);
-          uu[3] = qm::affine(gg[0].y, __uint_as_float(v[3]), bv[0].y);
-          uu[4] = qm::affine(gg[1].x, __uint_as_float(v[4]), bv[1].x);
-          uu[5] = qm::affine(gg[1].x, __uint_as_float(v[5]), bv[1].x);
-          uu[6] = qm::affine(gg[1].y, __uint_as_float(v[6]), bv[1].y);
-          uu[7] = qm::affine(gg[1].y, __uint_as_float(v[7]), bv[1].y);
+          uu[0] = qm::affine(gg[0].x, __uint_as_float(v[0]), gg[0].z);
+          uu[1] = qm::affine(gg[0].x, __uint_as_float(v[1]), gg[0].z);
+          uu[2] = qm::affine(gg[0].y, __uint_as_float(v[2]), gg[0].w);
+          uu[3] = qm::affine(gg[0].y, __uint_as_float(v[3]), gg[0].w);
+          uu[4] = qm::affine(gg[1].x, __uint_as_float(v[4]), gg[1].z);
+          uu[5] = qm::affine(gg[1].x, __uint_as_float(v[5]), gg[1].z);
+          uu[6] = qm::affine(gg[1].y, __uint_as_float(v[6]), gg[1].w);
+          uu[7] = qm::affine(gg[1].y, __uint_as_float(v[7]), gg[1].w);
           m0 = qm::max3_abs(m0, uu[0], uu[2]);
           m1 = qm::max3_abs(m1, uu[1], uu[3]);
-          if (lb + 1 < nb) {
+          if (2 * u + 1 < my_blocks) {                   // an odd last block: the spare columns hold no data
             m0 = qm::max3_abs(m0, uu[4], uu[6]);
             m1 = qm::max3_abs(m1, uu[5], uu[7]);
           }
-          tmem_st_16x256b_x2(tbuf + static_cast<uint32_t>(lb * kTok), uu);
-        }
-      };
-      if (nunits > 0) load(0, va, ga, ba);
-      for (int u = 0; u < nunits; u += 2) {
-        ptx::tmem_ld_wait();
-        if (u + 1 < nunits) load(u + 1, vb, gb, bb);
-        math(u, va, ga, ba);
-        if (u + 1 < nunits) {
+          tmem_st_16x256b_x2(tbuf + static_cast<uint32_t>(2 * u * kTok), uu);
+        };
+        load(0, va, ga);
+#pragma unroll
+        for (int u = 0; u < UPS; u += 2) {
           ptx::tmem_ld_wait();
-          if (u + 2 < nunits) load(u + 2, va, ga, ba);
-          math(u + 1, vb, gb, bb);
+          if (u + 1 < UPS) load(u + 1, vb, gb);
+          if (u < nunits) math(u, va, ga);
+          if (u + 1 < UPS) {
+            ptx::tmem_ld_wait();
+            if (u + 2 < UPS) load(u + 2, va, ga);
+            if (u + 1 < nunits) math(u + 1, vb, gb);
+          }
         }
+        ptx::tmem_st_wait();
       }
-      ptx::tmem_st_wait();
       // over r (lane bits 2..4) inside the warp; the 16 warps meet in shared memory
 #pragma unroll
       for (int o = 4; o < 32; o <<= 1) {
@@ -439,45 +441,47 @@ quantize_had_tc_kernel(const __grid_constant__ CUtensorMap tmap_x, const TcParam
     // ---- pass 2 of group gi: u back from tensor memory, round, pack whole bytes, stage
     auto pass2 = [&](int gi) {
       const uint32_t buf = static_cast<uint32_t>(gi) & 1u, phase = (static_cast<uint32_t>(gi) >> 1) & 1u;
-      const uint32_t tbuf = taddr0 + buf * kDCols;
-      uint8_t* tile = code_tile + buf * kCodeTile;
+      const uint32_t tbuf = taddr0 + buf * kDCols + static_cast<uint32_t>(bl0 * kTok);
+      uint8_t* tile = code_tile + buf * kCodeTile + bl0 * 64 + pair;
       ptx::mbar_wait(ptx::smem_u32(&bars->invfull[buf]), phase);
       const float inv0 = sm->inv[buf][2 * c], inv1 = sm->inv[buf][2 * c + 1];
       // the bulk stores of group gi - 2 have read this tile
       if (gi >= 2) ptx::mbar_wait(ptx::smem_u32(&bars->tempty[buf]), ((static_cast<uint32_t>(gi) >> 1) - 1u) & 1u);
-      uint32_t va[8], vb[8];
-      auto load = [&](int u, uint32_t (&v)[8]) {
-        tmem_ld_16x256b_x2(tbuf + static_cast<uint32_t>(min(unit_block(u), kMaxBlocks - 2) * kTok), v);
-      };
-      auto math = [&](int u, const uint32_t (&v)[8]) {
-        const int lb = unit_block(u);
-        if (lb < nb) {
-          // byte = (q[2j + 1] & 15) << 4 | (q[2j] & 15), both clamped to [-8, 7] by the pack
-          const uint32_t b0 = qm::pack2_sat(qm::code_int(__uint_as_float(v[2]), inv0), qm::code_int(__uint_as_float(v[0]), inv0), 0u);
-          const uint32_t b1 = qm::pack2_sat(qm::code_int(__uint_as_float(v[3]), inv1), qm::code_int(__uint_as_float(v[1]), inv1), 0u);
-          uint8_t* dst = tile + lb * 64 + jbyte;
-          dst[(2 * c) * kCodePitch] = static_cast<uint8_t>(b0);
-          dst[(2 * c + 1) * kCodePitch] = static_cast<uint8_t>(b1);
-          if (lb + 1 < nb) {
-            const uint32_t b2 = qm::pack2_sat(qm::code_int(__uint_as_float(v[6]), inv0), qm::code_int(__uint_as_float(v[4]), inv0), 0u);
-            const uint32_t b3 = qm::pack2_sat(qm::code_int(__uint_as_float(v[7]), inv1), qm::code_int(__uint_as_float(v[5]), inv1), 0u);
-            dst[64 + (2 * c) * kCodePitch] = static_cast<uint8_t>(b2);
-            dst[64 + (2 * c + 1) * kCodePitch] = static_cast<uint8_t>(b3);
-          }
+      auto math = [&](int u, const uint32_t (&vv)[8]) {
+        // byte = (q[2j + 1] & 15) << 4 | (q[2j] & 15), both clamped to [-8, 7] by the pack
+        const uint32_t b0 = qm::pack2_sat(qm::code_int(__uint_as_float(vv[2]), inv0), qm::code_int(__uint_as_float(vv[0]), inv0), 0u);
+        const uint32_t b1 = qm::pack2_sat(qm::code_int(__uint_as_float(vv[3]), inv1), qm::code_int(__uint_as_float(vv[1]), inv1), 0u);
+        uint8_t* dst = tile + 2 * u * 64;
+        dst[(2 * c) * kCodePitch] = static_cast<uint8_t>(b0);
+        dst[(2 * c + 1) * kCodePitch] = static_cast<uint8_t>(b1);
+        if (2 * u + 1 < my_blocks) {
+          const uint32_t b2 = qm::pack2_sat(qm::code_int(__uint_as_float(vv[6]), inv0), qm::code_int(__uint_as_float(vv[4]), inv0), 0u);
+          const uint32_t b3 = qm::pack2_sat(qm::code_int(__uint_as_float(vv[7]), inv1), qm::code_int(__uint_as_float(vv[5]), inv1), 0u);
+          dst[64 + (2 * c) * kCodePitch] = static_cast<uint8_t>(b2);
+          dst[64 + (2 * c + 1) * kCodePitch] = static_cast<uint8_t>(b3);
         }
       };
-      // slot by slot: both units of the slot into registers, the slot released to the MMAs of group
-      // gi + 2 (they run under the rounding work), then the math
-      for (int j = 0; j < nslots; ++j) {
-        load(2 * j, va);
-        load(2 * j + 1, vb);
+      // the warp's units in two chunks of registers; once the last loads have completed the slot is
+      // released to the MMAs of group gi + 2 (they run under the rest of the rounding work)
+      constexpr int kHalf = (UPS + 1) / 2;
+      uint32_t va[kHalf][8], vb[UPS - kHalf + 1][8];
+      if (nunits > 0) {
+#pragma unroll
+        for (int i = 0; i < kHalf; ++i) tmem_ld_16x256b_x2(tbuf + static_cast<uint32_t>(2 * i * kTok), va[i]);
         ptx::tmem_ld_wait();
-        ptx::tcgen05_fence_before();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&bars->dempty[buf][j]));
-        math(2 * j, va);
-        math(2 * j + 1, vb);
+#pragma unroll
+        for (int i = kHalf; i < UPS; ++i) tmem_ld_16x256b_x2(tbuf + static_cast<uint32_t>(2 * i * kTok), vb[i - kHalf]);
+#pragma unroll
+        for (int i = 0; i < kHalf; ++i)
+          if (i < nunits) math(i, va[i]);
+        ptx::tmem_ld_wait();
       }
+      ptx::tcgen05_fence_before();
+      __syncwarp();
+      if (lane == 0 && team < nslots) ptx::mbar_arrive(ptx::smem_u32(&bars->dempty[buf][team]));
+#pragma unroll
+      for (int i = kHalf; i < UPS; ++i)
+        if (i < nunits) math(i, vb[i - kHalf]);
       ptx::fence_proxy_async_smem();                    // this lane's tile bytes -> the bulk-copy engine
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&bars->tfull[buf]));
@@ -521,34 +525,10 @@ EncodeTiledFn tc_encode_fn() {
   return fn;
 }
 
-}  // namespace
-
-bool quantize_tc_supported(int K, int had_block) {
-  return had_block == kBlk && K % kBlk == 0 && K / kBlk <= kMaxBlocks * kMaxCluster;
-}
-
-cudaError_t launch_quantize_tc(const QuantLaunch& q) {
-  if (!quantize_tc_supported(q.K, q.had_block) || q.asym) return cudaErrorNotSupported;
-  EncodeTiledFn encode = tc_encode_fn();
-  if (encode == nullptr) return cudaErrorNotSupported;
-  // X as a 4-D tensor [2 halves of a block][K / 128 blocks][T tokens][64 channels]: a box lands in
-  // shared memory as [half][block][8 tokens x 128 bytes] -- for each half the 64 (block, token) rows
-  // of one K-major SWIZZLE_128B operand of tcgen05.mma
-  CUtensorMap tmap{};
-  const cuuint64_t dims[4] = {64, static_cast<cuuint64_t>(q.T), static_cast<cuuint64_t>(q.K / kBlk), 2};
-  const cuuint64_t strides[3] = {static_cast<cuuint64_t>(q.ldx) * 2, 256, 128};
-  const cuuint32_t box[4] = {64, kTok, kSB, 2};
-  const cuuint32_t estr[4] = {1, 1, 1, 1};
-  const CUresult r = encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(q.x), dims, strides,
-                            box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-
-  const int nblk = q.K / kBlk;
-  int C = 1;
-  while ((nblk + C - 1) / C > kMaxBlocks) C *= 2;
+template <int UPS>
+cudaError_t launch_ups(const QuantLaunch& q, const CUtensorMap& tmap, int nblk, int C) {
   static std::atomic<int> attr_smem[kMaxDevices];
-  const cudaError_t ea = ensure_dynamic_smem(quantize_had_tc_kernel, kTcSmemBytes, q.device, attr_smem);
+  const cudaError_t ea = ensure_dynamic_smem(quantize_had_tc_kernel<UPS>, kTcSmemBytes, q.device, attr_smem);
   if (ea != cudaSuccess) return ea;
   const int groups = (q.T + kTok - 1) / kTok;
 
@@ -581,13 +561,13 @@ cudaError_t launch_quantize_tc(const QuantLaunch& q) {
   // cluster that had to wait for a free GPC slot would start a whole wave late.  How many clusters
   // of C CTAs with this much shared memory fit depends on the GPC layout of the part (15 of 8 on a
   // B200, not 148 / 8 = 18): ask once per device and cluster size.
-  static std::atomic<int> max_clusters[kMaxDevices][4];
+  static std::atomic<int> max_clusters[kMaxDevices][4];   // per UPS instantiation
   const int ci = C == 1 ? 0 : C == 2 ? 1 : C == 4 ? 2 : 3;
   int fit = max_clusters[q.device][ci].load(std::memory_order_acquire);
   if (fit == 0) {
     cfg.gridDim = dim3(static_cast<unsigned>(q.num_sms / C * C), 1, 1);
     int n = 0;
-    if (cudaOccupancyMaxActiveClusters(&n, quantize_had_tc_kernel, &cfg) != cudaSuccess || n < 1) {
+    if (cudaOccupancyMaxActiveClusters(&n, quantize_had_tc_kernel<UPS>, &cfg) != cudaSuccess || n < 1) {
       (void)cudaGetLastError();
       n = q.num_sms / C > 2 ? q.num_sms / C - 2 : 1;
     }
@@ -596,7 +576,49 @@ cudaError_t launch_quantize_tc(const QuantLaunch& q) {
   }
   const int clusters = fit < groups ? fit : groups;
   cfg.gridDim = dim3(static_cast<unsigned>(clusters * C), 1, 1);
-  return cudaLaunchKernelEx(&cfg, quantize_had_tc_kernel, tmap, p);
+  return cudaLaunchKernelEx(&cfg, quantize_had_tc_kernel<UPS>, tmap, p);
+}
+
+}  // namespace
+
+bool quantize_tc_supported(int K, int had_block) {
+  return had_block == kBlk && K % kBlk == 0 && K / kBlk <= kMaxBlocks * kMaxCluster;
+}
+
+cudaError_t launch_quantize_tc(const QuantLaunch& q) {
+  if (!quantize_tc_supported(q.K, q.had_block) || q.asym) return cudaErrorNotSupported;
+  EncodeTiledFn encode = tc_encode_fn();
+  if (encode == nullptr) return cudaErrorNotSupported;
+  const int nblk = q.K / kBlk;
+  int C = 1;
+  while ((nblk + C - 1) / C > kMaxBlocks) C *= 2;
+  // a CTA's blocks (at most ceil(nblk / C)) in two slots of sb blocks, sb even: both epilogue teams
+  // get the same amount of work
+  const int per = (nblk + C - 1) / C;
+  const int sb = (((per + 1) / 2) + 1) / 2 * 2;
+  // X as a 4-D tensor [2 halves of a block][K / 128 blocks][T tokens][64 channels]: a box lands in
+  // shared memory as [half][block][8 tokens x 128 bytes] -- for each half the 64 (block, token) rows
+  // of one K-major SWIZZLE_128B operand of tcgen05.mma
+  CUtensorMap tmap{};
+  const cuuint64_t dims[4] = {64, static_cast<cuuint64_t>(q.T), static_cast<cuuint64_t>(q.K / kBlk), 2};
+  const cuuint64_t strides[3] = {static_cast<cuuint64_t>(q.ldx) * 2, 256, 128};
+  const cuuint32_t box[4] = {64, kTok, static_cast<cuuint32_t>(sb), 2};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const CUresult r = encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(q.x), dims, strides,
+                            box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+
+  switch (sb / 2) {
+    case 1: return launch_ups<1>(q, tmap, nblk, C);
+    case 2: return launch_ups<2>(q, tmap, nblk, C);
+    case 3: return launch_ups<3>(q, tmap, nblk, C);
+    case 4: return launch_ups<4>(q, tmap, nblk, C);
+    case 5: return launch_ups<5>(q, tmap, nblk, C);
+    case 6: return launch_ups<6>(q, tmap, nblk, C);
+    case 7: return launch_ups<7>(q, tmap, nblk, C);
+    default: return cudaErrorInvalidValue;
+  }
 }
 
 }  // namespace baseq
