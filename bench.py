@@ -39,6 +39,35 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
 
 
+def kernel_source_hash():
+    """sha256 (first 16 hex digits) over the CUDA sources of libbaseq: ties a stored ncu figure to the
+    build it was captured from (the GPU box has no .git)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2506_15689_b200", "csrc")
+    for fn in sorted(os.listdir(d)):
+        if fn.endswith((".cu", ".cuh")):
+            h.update(fn.encode())
+            h.update(open(os.path.join(d, fn), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def stored_traffic(kernel):
+    """dram bytes per launch of `kernel` from the ncu capture summarised in profiles/traffic.csv --
+    only if that capture was taken from THIS build (same kernel_source_hash), else None."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tpath):
+        return None, "no profiles/traffic.csv"
+    here = kernel_source_hash()
+    for ln in open(tpath).read().splitlines()[1:]:
+        f = ln.split(",")
+        if len(f) >= 4 and f[0] == kernel and f[1].startswith("average"):
+            if f[3].strip() == here:
+                return int(f[2]), "profiles/traffic.csv (ncu --set full, csrc hash %s)" % here
+            return None, "profiles/traffic.csv is from another build (csrc hash %s, this build %s)" % (f[3].strip(), here)
+    return None, "kernel not in profiles/traffic.csv"
+
+
 def step_plan(config):
     """Groups the config's layers by the activation they share: [(act, [layer specs])]."""
     plan, seen = [], {}
@@ -293,15 +322,9 @@ def run_gpu(args):
                   clocks["sm_mhz"] >= 0.95 * clocks["sm_max_mhz"])
     which = "burst" if at_max else "sustained"
     int8_peak = 2.0 * peaks["bf16_" + which]
-    traffic = None     # dram bytes per launch of the dominant kernel, from the ncu capture in profiles/
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(tpath):
-        for ln in open(tpath).read().splitlines()[1:]:
-            f = ln.split(",")
-            if f[0] == "w4a4_gemm_kernel" and f[1].startswith("average"):
-                traffic = int(f[2])
+    traffic, traffic_source = stored_traffic("w4a4_gemm_kernel")
     roofline = {"bound": "tensor", "kernel": "w4a4_gemm_kernel", "achieved": tops, "peak": int8_peak,
-                "unit": "TFLOP/s", "frac": tops / int8_peak, "traffic": traffic,
+                "unit": "TFLOP/s", "frac": tops / int8_peak, "traffic": traffic, "traffic_source": traffic_source,
                 "peak_source": "2 x %s bf16 %s (%s MEASURED_PEAKS.json; int8:bf16 nominal ratio 2; "
                                "SM clock %s of %s MHz during the timed region)"
                                % (peaks["bf16_" + which], which, peaks["source"], clocks.get("sm_mhz"),
@@ -317,6 +340,67 @@ def run_gpu(args):
     per_layer = [{"kernel": kd[0], "name": kd[1], "ms": float(per_kernel[i]),
                   "rate": float(kd[2] / (per_kernel[i] * 1e-3) / (1e12 if kd[0] == "gemm" else 1e9)),
                   "rate_unit": "TOP/s" if kd[0] == "gemm" else "GB/s"} for i, kd in enumerate(kernels)]
+
+    # ---- sustained leg: the same step back to back for >= 2 s (the 20-step region above lasts a few
+    # ms at the full clock -- a burst figure; after ~100 ms the part settles at its power cap), no
+    # events between the kernels (dependent launches overlap), its own clock record, and a FIXED
+    # denominator: 2 x the bf16 figure MEASURED_PEAKS.json took the same way (seconds-long loop)
+    sustained = None
+    if not args.no_sustained:
+        s2 = ClockSampler(local_rank)
+        s2.start()
+        torch.cuda.synchronize()
+        n_done, t_wall = 0, time.time()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        while True:
+            for _ in range(200):
+                step(None)
+            n_done += 200
+            torch.cuda.synchronize()
+            if time.time() - t_wall >= args.sustain_seconds:
+                break
+        e1.record()
+        torch.cuda.synchronize()
+        c2 = s2.stop()
+        sms = max_over_ranks(e0.elapsed_time(e1), ws, torch.device("cuda", local_rank)) / n_done
+        share = gemm_ms / per_kernel.sum()
+        stops = gemm_ops / (sms * share * 1e-3) / 1e12
+        sustained = {"seconds": time.time() - t_wall, "steps": n_done, "ms_per_step": sms,
+                     "tokens_per_s": ws * T / (sms * 1e-3), "clocks": c2,
+                     "gemm_TOP_per_s": stops, "gemm_share_assumed": share,
+                     "frac_of_2x_bf16_sustained": stops / (2.0 * peaks["bf16_sustained"]),
+                     "frac_of_nominal_4500": stops / 4500.0,
+                     "note": "includes a torch.cuda.synchronize every 200 steps; GEMM rate = 2 T N K of the step's "
+                             "GEMMs over the step time x the GEMM share of the event-timed region"}
+
+    # ---- NEXT-2: the same step with the online Hadamard on the tensor cores (tolerance parity)
+    tc_step = None
+    if any(acts[a]["params"].had_block == 128 for a, _ in plan):
+        def step_tc():
+            for act, specs in plan:
+                a = acts[act]
+                if a["params"].had_block == 128:
+                    bq.quantize_act_tc(a["x"], a["params"], a["codes"], a["scales"])
+                else:
+                    bq.quantize_act(a["x"], a["params"], a["codes"], a["scales"])
+                for sp in specs:
+                    bq.w4a4_gemm(a["codes"], a["scales"], layers[sp.name]["pw"], layers[sp.name]["y"])
+        for _ in range(3):
+            step_tc()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            step_tc()
+        e1.record()
+        torch.cuda.synchronize()
+        tms = e0.elapsed_time(e1) / args.steps
+        tc_step = {"ms_per_step": tms, "tokens_per_s": ws * T / (tms * 1e-3),
+                   "note": "baseq_quantize_act_tc + baseq_w4a4_gemm; codes inside the band of DESIGN.md 6.9, not bit-equal "
+                           "to the butterfly contract (quantizer_cold[].tensor_core_hadamard)"}
+        step()      # leave the contract's codes / outputs in the buffers for the checks below
+        torch.cuda.synchronize()
 
     # ---- the fused variant (a10) on the same layers, reported beside the two-kernel path
     fused = run_fused(args, bq, torch, plan, acts, layers, T)
@@ -334,7 +418,8 @@ def run_gpu(args):
             "dtype": "int4xint4->int32 (tcgen05 kind::i8); fp32 quantizer; bf16 out",
             "data": "synthetic", "config": workload_config(config), "clocks": clocks,
             "e2e": e2e, "gpu_launches": nk * args.steps, "roofline": roofline,
-            "roofline_quantizer": roofline_q, "kernels": per_layer, "fused_variant": fused,
+            "roofline_quantizer": roofline_q, "kernels": per_layer, "sustained": sustained, "tensor_core_hadamard_step": tc_step,
+            "kernel_source_hash": kernel_source_hash(), "fused_variant": fused,
             "asym_variant": asym, "kv_quantizer": kv, "quantizer_cold": qcold,
             "decode_shapes": decode}
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
@@ -435,10 +520,44 @@ def run_kv(args, bq, torch, T, hbm_gbs):
     return out
 
 
+def graph_time(torch, fn, n_calls, reps):
+    """Device time per call of fn(k), k = 0 .. n_calls - 1, replayed from a CUDA graph: the host's
+    launch path (ctypes + cudaLaunchKernelEx, ~8 us per call) is longer than the short kernels, so an
+    eager loop would time the CPU.  Returns ms per call."""
+    for k in range(n_calls):
+        fn(k)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            for k in range(n_calls):
+                fn(k)
+    torch.cuda.current_stream().wait_stream(side)
+    graph.replay()
+    torch.cuda.synchronize()
+    best = None
+    for _ in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _r in range(reps):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / (reps * n_calls)
+        best = ms if best is None else min(best, ms)
+    del graph
+    return best
+
+
 def run_quant_cold(args, bq, torch, plan, acts, T, hbm_gbs):
     """the quantiser timed alone, cold -- back-to-back launches rotating over enough
     (X, codes) buffer sets that the footprint exceeds 2 x L2 -- next to the in-step figure of
-    `roofline_quantizer` (which includes the gap after the preceding GEMM)."""
+    `roofline_quantizer` (which includes the gap after the preceding GEMM).  Timed as a CUDA graph of
+    the rotation (device time; the eager loop's figure, which at these sizes measures the host's
+    launch path, is kept beside it).  Activations with the online Hadamard are also run through the
+    tensor-core mode (NEXT-2, baseq_quantize_act_tc; tolerance parity)."""
     steps = max(10, min(args.steps, 40))
     out = []
     for act, _specs in plan:
@@ -457,10 +576,25 @@ def run_quant_cold(args, bq, torch, plan, acts, T, hbm_gbs):
             bq.quantize_act(xs[k % nbuf], a["params"], *outs[k % nbuf])
         e1.record()
         torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / steps
+        eager_ms = e0.elapsed_time(e1) / steps
+        ms = graph_time(torch, lambda k: bq.quantize_act(xs[k], a["params"], *outs[k]), nbuf, max(2, 40 // nbuf))
         gbs = by / (ms * 1e-3) / 1e9
-        out.append({"name": act, "T": T, "K": K, "ms": ms, "GB_per_s": gbs,
-                    "frac_of_measured_hbm": gbs / hbm_gbs, "buffers_rotated": nbuf})
+        row = {"name": act, "T": T, "K": K, "ms": ms, "GB_per_s": gbs, "frac_of_measured_hbm": gbs / hbm_gbs,
+               "frac_of_nominal_8000": gbs / 8000.0, "buffers_rotated": nbuf, "timed_as": "CUDA graph of the rotation",
+               "eager_ms": eager_ms}
+        if a["params"].had_block == 128:
+            tms = graph_time(torch, lambda k: bq.quantize_act_tc(xs[k], a["params"], *outs[k]), nbuf, max(2, 40 // nbuf))
+            c_ref, s_ref = bq.quantize_act(xs[0], a["params"])
+            c_tc, s_tc = bq.quantize_act_tc(xs[0], a["params"])
+            torch.cuda.synchronize()
+            row["tensor_core_hadamard"] = {
+                "kernel": "quantize_had_tc_kernel (tcgen05 kind::f16, NEXT-2)", "ms": tms,
+                "GB_per_s": by / (tms * 1e-3) / 1e9, "frac_of_measured_hbm": by / (tms * 1e-3) / 1e9 / hbm_gbs,
+                "speedup_over_butterfly_contract": ms / tms,
+                "code_bytes_differing_from_contract": float((c_ref != c_tc).float().mean().item()),
+                "max_rel_scale_difference": float(((s_ref - s_tc).abs() / s_ref).max().item()),
+                "parity": "tolerance band of DESIGN.md 6.9 (tests/test_gpu_parity.py::test_quantizer_tc_*)"}
+        out.append(row)
         del xs, outs
     return out
 
@@ -662,6 +796,8 @@ def main():
     ap.add_argument("--impl", default="baseq", choices=["baseq", "reference"])
     ap.add_argument("--config", default="c3", choices=sorted(CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the >= 2 s sustained leg")
+    ap.add_argument("--sustain-seconds", type=float, default=2.5)
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
