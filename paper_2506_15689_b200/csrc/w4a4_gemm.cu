@@ -59,10 +59,7 @@ static_assert(BN % 32 == 0 && BN <= 256, "UMMA N");
 constexpr int kSetsMax = 2;             // A and B warp sets alternate k-blocks: one warp's serial
                                         // chain per k-block (two try_waits, LDS, expand, store,
                                         // fence, arrive: 400-700 clk) exceeds the 384 clk MMA time
-constexpr int kProducerWarp = 0;        // A operand (tensor-map TMA; idle in the fused variant)
-constexpr int kProducerWarpB = 2;       // B operand (bulk TMA)
-constexpr int kMmaWarp = 1;
-constexpr int kEpiWarp0 = 4;            // epilogue warps start here (warp % 4 = TMEM lane quarter)
+constexpr int kEpiWarp0 = 0;            // epilogue warps start here (warp % 4 = TMEM lane quarter)
 constexpr int kNumUnpackWarps = 4;      // per set
 constexpr int kAStageBytes = BM * BK;   // fused variant: int8 A operand stage in shared memory
 
@@ -85,7 +82,13 @@ struct Cfg {
   static constexpr int kSets = FUSED ? 1 : kSetsMax;
   static constexpr int kAWarp0 = kEpiWarp0 + kEpiWarps;     // 8 A warps in both variants
   static constexpr int kUnpackWarp0 = kAWarp0 + 8;
-  static constexpr int kThreads = 32 * (kUnpackWarp0 + kNumUnpackWarps * kSets);
+  // the single-lane roles sit ABOVE the data warps: the warp scheduler of a sub-partition favours the
+  // higher warp id among eligible warps, and a late TMA issue or MMA issue stalls everybody else
+  static constexpr int kRoleWarp0 = kUnpackWarp0 + kNumUnpackWarps * kSets;
+  static constexpr int kProducerWarp = kRoleWarp0;        // A operand (tensor-map TMA; idle in the fused variant)
+  static constexpr int kProducerWarpB = kRoleWarp0 + 1;   // B operand (bulk TMA)
+  static constexpr int kMmaWarp = kRoleWarp0 + 3;
+  static constexpr int kThreads = 32 * (kRoleWarp0 + 4);
   static constexpr int kBRows = BN / CG;                   // weight rows staged per CTA
   static constexpr int kPackedB = kBRows * BK / 2;
   static constexpr int kPackedAArea = FUSED ? 0 : kPackedA;
@@ -227,6 +230,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
   constexpr int kSets = C::kSets;
   constexpr int kAWarp0 = C::kAWarp0;
   constexpr int kUnpackWarp0 = C::kUnpackWarp0;
+  constexpr int kProducerWarp = C::kProducerWarp, kProducerWarpB = C::kProducerWarpB, kMmaWarp = C::kMmaWarp;
   extern __shared__ uint8_t smem_raw[];
   // SWIZZLE_128B operands need 1024-byte alignment
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
