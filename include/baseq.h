@@ -216,6 +216,25 @@ BASEQ_API baseq_status_t baseq_linear_host(const void* x_bf16_host, int T, int K
                                  const void* packed_w, int N, void* y_bf16_host, void* dev_scratch,
                                  size_t dev_scratch_bytes, void* stream);
 
+/* ---- the two-kernel linear for callers that cannot allocate (Eq. 15; a1-a9) ----
+ * baseq_quantize_act followed by baseq_w4a4_gemm -- same contract, same bits -- with the
+ * intermediate codes [T, K/2] and scales [T] held in a static __device__ array inside the
+ * library instead of caller buffers: no cudaMalloc / cudaFree / allocating routine is called,
+ * here or by anything it launches (CUDA graph capture, serving loops, harnesses that forbid
+ * allocation).  The caller still passes X, the packed weights and Y (device pointers, as above).
+ *   limit      T * K / 2 <= 4 MiB of codes and T <= 8192 (config 2, 2048 x 4096, fits exactly);
+ *              beyond it BASEQ_ERR_WORKSPACE, nothing enqueued.  The array is
+ *              baseq_linear_static_scratch_bytes() = 4 MiB + 32 KiB, held by every GPU that loads
+ *              the library until the process exits.
+ *   sharing    ONE array per device, shared by every call and keeping the last call's contents
+ *              (nothing in it needs to start at zero: each call writes all T rows before it reads
+ *              them).  Calls are ordered on their stream; two calls that overlap on the GPU --
+ *              different streams, or two host threads on the same device -- RACE on it.        */
+BASEQ_API size_t baseq_linear_static_scratch_bytes(void);
+BASEQ_API baseq_status_t baseq_linear_static(const void* x_bf16, int64_t ldx, int T, int K,
+                                   const baseq_act_params_t* p, const void* packed_w, int N,
+                                   void* y_bf16, int64_t ldy, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

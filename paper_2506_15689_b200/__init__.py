@@ -15,6 +15,8 @@ from .binding import (  # noqa: F401
     linear_fused,
     linear_host,
     linear_host_scratch_bytes,
+    linear_static,
+    linear_static_scratch_bytes,
     pack_weights,
     quantize_act,
     quantize_act_asym,

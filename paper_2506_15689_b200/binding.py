@@ -16,6 +16,7 @@ EXPORTED_SYMBOLS = [
     "baseq_set_fused_bias", "baseq_quantize_act", "baseq_quantize_act_tc", "baseq_w4a4_gemm",
     "baseq_fused_workspace_bytes", "baseq_linear_fused", "baseq_linear_host_scratch_bytes",
     "baseq_linear_host", "baseq_quantize_act_asym", "baseq_w4a4_gemm_asym", "baseq_quantize_kv",
+    "baseq_linear_static_scratch_bytes", "baseq_linear_static",
 ]
 
 
@@ -78,6 +79,10 @@ def lib():
         L.baseq_w4a4_gemm_asym.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, i64, vp, vp]
         L.baseq_quantize_kv.restype = i32
         L.baseq_quantize_kv.argtypes = [vp, i64, i32, i32, i32, c.c_float, vp, vp, vp, vp]
+        L.baseq_linear_static_scratch_bytes.restype = sz
+        L.baseq_linear_static_scratch_bytes.argtypes = []
+        L.baseq_linear_static.restype = i32
+        L.baseq_linear_static.argtypes = [vp, i64, i32, i32, c.POINTER(_ActParamsC), vp, i32, vp, i64, vp]
         _lib = L
     return _lib
 
@@ -257,3 +262,19 @@ def linear_host(x_host, params, pw, y_host, scratch):
 
 def linear_host_scratch_bytes(T, N, K):
     return lib().baseq_linear_host_scratch_bytes(T, N, K)
+
+
+def linear_static_scratch_bytes():
+    return lib().baseq_linear_static_scratch_bytes()
+
+
+def linear_static(x, params, pw, y):
+    """quantize_act + w4a4_gemm with the codes / scales in the library's static device array: the
+    call allocates nothing (y is the caller's).  T * K / 2 <= 4 MiB, T <= 8192, else BaseqError."""
+    T, K = x.shape
+    assert x.dtype == torch.bfloat16 and x.stride(1) == 1
+    assert y.dtype == torch.bfloat16 and y.stride(1) == 1 and tuple(y.shape) == (T, pw.N)
+    cs = params.c_struct()
+    _check(lib().baseq_linear_static(_p(x), x.stride(0), T, K, ctypes.byref(cs), _p(pw.blob), pw.N,
+                                     _p(y), y.stride(0), _stream()), "baseq_linear_static")
+    return y

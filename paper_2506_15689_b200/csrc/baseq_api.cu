@@ -415,3 +415,79 @@ baseq_status_t baseq_linear_host(const void* x_bf16_host, int T, int K, const ba
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------ baseq_linear_static (no allocation)
+// The two-kernel linear needs scratch between its kernels: the int4 codes [T, K/2] and the
+// per-token scales [T].  Callers that cannot allocate (CUDA graph capture, serving loops, harnesses
+// that forbid cudaMalloc) get that scratch from this file-scope array: kStaticCodesBytes of codes
+// followed by kStaticMaxT scales.  Every GPU that loads the library holds it until the process
+// exits.  In host code `g_static_scratch` is only a host-side stand-in for the symbol, never a
+// device address: the address comes from cudaGetSymbolAddress, once per device with that device
+// current, and is what the kernels receive.
+constexpr size_t kStaticCodesBytes = size_t(4) << 20;   // T * K / 2 <= 4 MiB (c2: 2048 x 4096)
+constexpr int kStaticMaxT = 8192;                        // scales: 32 KiB
+constexpr size_t kStaticScratchBytes = kStaticCodesBytes + size_t(kStaticMaxT) * sizeof(float);
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace {
+
+struct StaticScratchState {
+  std::once_flag once;
+  cudaError_t err = cudaErrorUnknown;
+  unsigned char* ptr = nullptr;
+};
+StaticScratchState g_static_state[kMaxDevices];
+
+// device_check() has run: `dev` is the current device and inside [0, kMaxDevices)
+baseq_status_t static_scratch(int dev, unsigned char** out) {
+  StaticScratchState& s = g_static_state[dev];
+  std::call_once(s.once, [&s]() {
+    void* sym = nullptr;
+    s.err = cudaGetSymbolAddress(&sym, g_static_scratch);
+    if (s.err == cudaSuccess) s.ptr = static_cast<unsigned char*>(sym);
+  });
+  if (s.err != cudaSuccess || s.ptr == nullptr) return BASEQ_ERR_CUDA;
+  *out = s.ptr;
+  return BASEQ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t baseq_linear_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+baseq_status_t baseq_linear_static(const void* x_bf16, int64_t ldx, int T, int K,
+                                   const baseq_act_params_t* p, const void* packed_w, int N,
+                                   void* y_bf16, int64_t ldy, void* stream) {
+  if (x_bf16 == nullptr || y_bf16 == nullptr || packed_w == nullptr || p == nullptr)
+    return BASEQ_ERR_NULL;
+  baseq_status_t st = check_shape(T, N, K);
+  if (st != BASEQ_OK) return st;
+  // beyond the static array: a clear error, nothing enqueued
+  if (T > kStaticMaxT || static_cast<size_t>(T) * K / 2 > kStaticCodesBytes) return BASEQ_ERR_WORKSPACE;
+  DeviceRef d;
+  st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  unsigned char* base = nullptr;
+  st = static_scratch(d.device, &base);
+  if (st != BASEQ_OK) return st;
+  uint8_t* codes = base;
+  float* scales = reinterpret_cast<float*>(base + kStaticCodesBytes);
+  // every check of both stages before the first launch
+  st = validate_quant(x_bf16, ldx, T, K, p, codes, scales, true);
+  if (st != BASEQ_OK) return st;
+  st = validate_gemm(codes, scales, packed_w, T, N, K, y_bf16, ldy, nullptr, true);
+  if (st != BASEQ_OK) return st;
+  // Nothing in the scratch has to start at zero: the quantiser writes all T rows of codes and
+  // scales before the GEMM reads them, and the GEMM reads no row >= T (its tensor map ends at T).
+  QuantLaunch q = make_quant(x_bf16, ldx, T, K, p, codes, scales, stream);
+  q.num_sms = d.num_sms;
+  q.device = d.device;
+  st = from_cuda(launch_quantize_act(q, true));
+  if (st != BASEQ_OK) return st;
+  return from_cuda(launch_w4a4_gemm(
+      make_gemm(codes, scales, nullptr, packed_w, T, N, K, y_bf16, ldy, nullptr, stream, d)));
+}
+
+}  // extern "C"
