@@ -191,13 +191,20 @@ BASEQ_API baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int 
                                            int head_dim, float alpha, uint8_t* codes, float* scales,
                                            float* zeros, void* stream);
 
-/* ---- fused variant: quantise inside the GEMM producer; int4 codes never reach HBM ----
- * A per-token absmax pre-pass writes scales_out, then one GEMM kernel whose producer warps read
- * bf16 X tiles, apply Hadamard / scale / bias / round with the known per-token scale and write
- * int8 operands straight to shared memory.  Same contract and the same bits as
- * baseq_quantize_act followed by baseq_w4a4_gemm.
- *   workspace / workspace_bytes  scratch of at least baseq_fused_workspace_bytes(T, N, K)
- *   codes_dump   optional [T, K/2] copy of the codes the producer computed (parity runs), or NULL
+/* ---- fused variant (a10): quantiser and GEMM in ONE launch ----
+ * Four extra warps per CTA of the GEMM kernel quantise X in the background, one token row per
+ * warp, with the arithmetic of baseq_quantize_act; their codes go to `workspace` (the size of the
+ * codes, [T, K/2], resident in L2 for the shapes that fit it) and a counter per 128-row group tells
+ * the GEMM's TMA producers when a group is complete; tiles are walked M-major so the first wave
+ * needs the first one or two 256-row strips only.  No kernel boundary between quantiser and GEMM;
+ * the same contract and the same bits as baseq_quantize_act followed by baseq_w4a4_gemm.
+ * had_block: 0 or any power of two <= 256 dividing K (128 and 0 at full speed).
+ *   workspace / workspace_bytes  device scratch of at least baseq_fused_workspace_bytes(T, N, K)
+ *                = 256-byte-rounded counters + T * K / 2 bytes, 256-byte aligned; its contents on
+ *                entry do not matter (the call clears its counters on the stream first), it may
+ *                be reused by the next call on the same stream, and two calls that overlap on the
+ *                GPU must not share it
+ *   codes_dump   optional [T, K/2]: the codes are written there instead of the workspace, or NULL
  *   scales_out   [T] required                                                                */
 BASEQ_API size_t baseq_fused_workspace_bytes(int T, int N, int K);
 BASEQ_API baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,

@@ -233,16 +233,19 @@ def linear(x, params, pw, y=None):
     return w4a4_gemm(codes, scales, pw, y)
 
 
-def linear_fused(x, params, pw, y=None, codes_dump=None, acc_dump=None, scales=None):
-    """Fused variant: absmax pre-pass + quantise-in-producer GEMM."""
+def linear_fused(x, params, pw, y=None, codes_dump=None, acc_dump=None, scales=None, workspace=None):
+    """Fused variant: one launch, background quantiser warps inside the GEMM kernel.  `workspace`
+    (uint8, >= baseq_fused_workspace_bytes) may be reused between calls; allocated here if None."""
     T, K = x.shape
     L = lib()
     if y is None:
         y = torch.empty((T, pw.N), dtype=torch.bfloat16, device=x.device)
     if scales is None:
         scales = torch.empty((T,), dtype=torch.float32, device=x.device)
-    wsb = L.baseq_fused_workspace_bytes(T, pw.N, K)
-    ws = torch.empty(max(wsb, 256), dtype=torch.uint8, device=x.device)
+    ws = workspace
+    if ws is None:
+        ws = torch.empty(max(L.baseq_fused_workspace_bytes(T, pw.N, K), 256), dtype=torch.uint8,
+                         device=x.device)
     cs = params.c_struct()
     _check(L.baseq_linear_fused(_p(x), x.stride(0), T, K, ctypes.byref(cs), _p(pw.blob), pw.N,
                                 _p(y), y.stride(0), _p(ws), ws.numel(), _p(codes_dump), _p(scales),

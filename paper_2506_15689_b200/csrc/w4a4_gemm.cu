@@ -22,9 +22,10 @@
 //                 k-block into one of two BN-column TMEM accumulators; commits multicast to both CTAs
 //   warps 4-11    epilogue: tcgen05.ld -> dequant (+ fused bias) -> bf16 -> global; overlaps the
 //                 next tile's main loop through the second accumulator
-//   warps 12-19   A: LDS -> x16 expand -> tcgen05.st (two sets alternate k-blocks); in the fused
-//                 variant these eight warps quantise bf16 X instead (quant_math.cuh)
+//   warps 12-19   A: LDS -> x16 expand -> tcgen05.st (two sets alternate k-blocks)
 //   warps 20-27   B: packed int4 -> int8 into SWIZZLE_128B K-major stages (two sets)
+//   warps 28-31   fused variant (a10) only: background quantiser, one token row per warp
+//                 (quant_math.cuh), codes into an L2-resident workspace, per-128-row ready counters
 //
 // x16 unpack: for a 32-bit word w holding 8 two's-complement nibbles,
 //   lo = (w << 4) & 0xF0F0F0F0   -> 4 signed bytes = 16 * (even-k codes)
@@ -56,52 +57,53 @@ constexpr int kPackedA = BM * BK / 2;    // 8 KB of packed codes per CTA and k-b
 static_assert(kACol0 + kStages * (BK / 4) <= kTmemCols, "TMEM budget");
 static_assert(BN % 32 == 0 && BN <= 256, "UMMA N");
 
-constexpr int kSetsMax = 2;             // A and B warp sets alternate k-blocks: one warp's serial
+constexpr int kSets = 2;                // A and B warp sets alternate k-blocks: one warp's serial
                                         // chain per k-block (two try_waits, LDS, expand, store,
                                         // fence, arrive: 400-700 clk) exceeds the 384 clk MMA time
-constexpr int kEpiWarp0 = 0;            // epilogue warps start here (warp % 4 = TMEM lane quarter)
 constexpr int kNumUnpackWarps = 4;      // per set
-constexpr int kAStageBytes = BM * BK;   // fused variant: int8 A operand stage in shared memory
 
-// A tile belongs to a CTA pair (cta_group::2, M = 256).  FUSED = quantise-in-producer variant
-// (a10): the eight A warps read bf16 X, quantise with the per-token scale and write the int8
-// operand to SHARED memory (any thread -> element mapping is allowed there; the Hadamard needs 16
-// lanes per 128 channels), and the MMA takes both operands from shared memory (.ss form).
+// A tile belongs to a CTA pair (cta_group::2, M = 256).  FUSED = the single-launch variant (a10):
+// four more warps quantise bf16 X in the background -- one token row per warp, the same
+// quant_math.cuh contract as the stand-alone quantiser -- into a workspace the size of the codes
+// that lives in L2, raise a counter per 128-row group, and the A producer of a tile waits for its
+// group's counter before it issues the tile's first TMA load.  Tiles are walked M-major there, so
+// that the first wave needs the first one or two 256-row strips only.
 constexpr int CG = 2;                   // CTAs per tile
+constexpr int kQuantWarps = 4;          // fused variant: background quantiser warps per CTA
 template <bool FUSED>
 struct Cfg {
   // per-tile column operands of the epilogue (s_w, fb, wsum), one copy per accumulator stage
   static constexpr int kColParamBytes = kAccStages * 3 * BN * 4;
-  // [barriers 256 | column operands | pad] then, unfused only, the Y staging tiles of the TMA-store
-  // epilogue: per epilogue warp 32 rows x BN/2 columns of bf16 as 3 boxes of 32 rows x 64 bytes
+  // [barriers 256 | column operands | pad] then the Y staging tiles of the TMA-store epilogue: per
+  // epilogue warp 32 rows x BN/2 columns of bf16 as 3 boxes of 32 rows x 64 bytes
   static constexpr int kTailBytes = (256 + kColParamBytes + 1023) / 1024 * 1024;
-  static constexpr bool kTmaStore = !FUSED;
   static constexpr int kStoreWarpBytes = 32 * (BN / 2) * 2;
-  static constexpr int kStoreBytes = kTmaStore ? (FUSED ? 4 : 8) * kStoreWarpBytes : 0;
-  static constexpr int kEpiWarps = FUSED ? 4 : 8;           // x 32 rows; 2 column halves when 8
-  static constexpr int kSets = FUSED ? 1 : kSetsMax;
-  static constexpr int kAWarp0 = kEpiWarp0 + kEpiWarps;     // 8 A warps in both variants
+  static constexpr int kEpiWarps = 8;                       // x 32 rows; 2 column halves
+  static constexpr int kStoreBytes = kEpiWarps * kStoreWarpBytes;
+  // fused: the quantiser warps take the LOWEST warp ids (the scheduler of a sub-partition favours
+  // the higher id among eligible warps: background work must never beat a GEMM role to an issue slot)
+  static constexpr int kQuantWarp0 = 0;
+  static constexpr int kEpiWarp0 = FUSED ? kQuantWarps : 0;   // epilogue: warp % 4 = TMEM lane quarter
+  static constexpr int kAWarp0 = kEpiWarp0 + kEpiWarps;     // 8 A warps
   static constexpr int kUnpackWarp0 = kAWarp0 + 8;
   // the single-lane roles sit ABOVE the data warps: the warp scheduler of a sub-partition favours the
   // higher warp id among eligible warps, and a late TMA issue or MMA issue stalls everybody else
   static constexpr int kRoleWarp0 = kUnpackWarp0 + kNumUnpackWarps * kSets;
-  static constexpr int kProducerWarp = kRoleWarp0;        // A operand (tensor-map TMA; idle in the fused variant)
+  static constexpr int kProducerWarp = kRoleWarp0;        // A operand (tensor-map TMA)
   static constexpr int kProducerWarpB = kRoleWarp0 + 1;   // B operand (bulk TMA)
   static constexpr int kMmaWarp = kRoleWarp0 + 3;
-  static constexpr int kThreads = 32 * (kRoleWarp0 + 4);
+  static constexpr int kThreads = 32 * (kRoleWarp0 + 4);      // 896, fused 1024
   static constexpr int kBRows = BN / CG;                   // weight rows staged per CTA
   static constexpr int kPackedB = kBRows * BK / 2;
-  static constexpr int kPackedAArea = FUSED ? 0 : kPackedA;
-  static constexpr int kPackedStage = kPackedAArea + kPackedB;   // unfused: multiple of 1024
+  static constexpr int kPackedStage = kPackedA + kPackedB;   // multiple of 1024
   static constexpr int kUnpackedStage = kBRows * BK;
-  static constexpr int kAOperand = FUSED ? kStages * kAStageBytes : 0;
-  static constexpr int kPFullCount = FUSED ? 1 : 2;
-  static constexpr int kPEmptyCount = FUSED ? kNumUnpackWarps : kNumUnpackWarps + 4;
-  static constexpr int kFullCount = CG * ((FUSED ? 8 : 4) + kNumUnpackWarps);
+  static constexpr int kPFullCount = 2;
+  static constexpr int kPEmptyCount = kNumUnpackWarps + 4;
+  static constexpr int kFullCount = CG * (4 + kNumUnpackWarps);
   static constexpr int kTemptyCount = CG * kEpiWarps;
   static constexpr int kPStages = kPStagesMax;
   static constexpr int kSmemBytes =
-      1024 + kAOperand + kStages * kUnpackedStage + kPStages * kPackedStage + kTailBytes + kStoreBytes;
+      1024 + kStages * kUnpackedStage + kPStages * kPackedStage + kTailBytes + kStoreBytes;
   static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
 };
 
@@ -132,12 +134,14 @@ struct GemmParams {
   // fused variant only
   const uint4* x;           // bf16 [T, ldx] viewed as 16-byte vectors
   int64_t ldxv;             // ldx / 8
-  float gamma;
+  float alpha, gamma;
   const float* sa;
   const float* bvec;
   int had_block;
   float had_scale;
-  uint32_t* codes_dump;     // optional [T, K/8] words of 8 nibbles
+  uint32_t* codes_out;      // [T, K/8] words of 8 nibbles: the workspace (or the caller's codes_dump)
+  float* scales_out;        // [T] (= scales)
+  unsigned int* ready;      // [ceil(T / 128)] rows quantised per 128-row group, zero at launch
 };
 
 __device__ __forceinline__ void advance(int& stage, uint32_t& phase, int n) {
@@ -218,6 +222,80 @@ __device__ __forceinline__ void dequant_bracket_asym(int32_t raw, float st256, f
   lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
 }
 
+// ------------------------------------------------------------------------------ background quantiser
+// One pass (PASS 0: absmax; PASS 1: round, clamp, pack, store) of a quantiser warp over kQC vector
+// steps of its row, lane l owning vectors l, l + 32, ....  ONE BASIC BLOCK by construction -- no
+// branch, idle lanes and steps beyond the row are clamped to the row's last vector and masked where
+// the values are used -- because ptxas tracks loads that cross a branch with a single scoreboard, and
+// then the wait for ring slot d also waits for the refill issued one step earlier (measured: one
+// memory round trip per step).  In straight-line code the kQD-deep register ring {x vector, its 8 b
+// values} is a true software pipeline.  HAD: 0 = no rotation, 128 = block-128 Hadamard (compile
+// time: qm::hadamard8 unrolls to 32 shuffles); everything else takes the generic step below.
+constexpr int kQD = 4;     // ring slots = loads in flight per lane: x + 2 x b per slot
+constexpr int kQC = 8;     // vector steps per chunk
+template <int PASS, int HAD>
+__device__ __forceinline__ void quant_chunk(const uint4* __restrict__ xr, const float* __restrict__ bvec,
+                                            float gamma, float had_scale, int lane, int nv, int nvl,
+                                            int c0, float inv, float& m, uint32_t* __restrict__ cr) {
+  uint4 sx[kQD];
+  float4 sb0[kQD], sb1[kQD];
+  auto issue = [&](int d, int j) {
+    int i = lane + 32 * j;
+    i = i < nv ? i : nv - 1;
+    sx[d] = __ldg(xr + i);
+    sb0[d] = __ldg(reinterpret_cast<const float4*>(bvec) + 2 * i);
+    sb1[d] = __ldg(reinterpret_cast<const float4*>(bvec) + 2 * i + 1);
+  };
+#pragma unroll
+  for (int d = 0; d < kQD; ++d) issue(d, c0 + d);
+  if (PASS == 0) {
+    // the chunk after the next one, towards L2: the ring's own depth covers an L2 hit, not an HBM miss
+    const int jp = c0 + 2 * kQC + (lane >> 2);            // 8 steps x 4 lines of 128 bytes
+    if (jp < nvl) ptx::prefetch_l2(reinterpret_cast<const uint8_t*>(xr + 32 * jp) + 128 * (lane & 3));
+  }
+#pragma unroll
+  for (int t = 0; t < kQC; ++t) {
+    const int d = t % kQD;
+    const int j = c0 + t;
+    const int i = lane + 32 * j;
+    const bool valid = j < nvl && i < nv;
+    float f[8], u[8];
+    qm::unpack8(sx[d], f);
+    if (HAD != 0) qm::hadamard8(f, HAD, had_scale, lane);
+    const float bb[8] = {sb0[d].x, sb0[d].y, sb0[d].z, sb0[d].w, sb1[d].x, sb1[d].y, sb1[d].z, sb1[d].w};
+#pragma unroll
+    for (int e = 0; e < 8; ++e) u[e] = qm::affine(gamma, f[e], bb[e]);
+    if (PASS == 0) {
+      const float mm = qm::absmax8(m, u);
+      m = valid ? mm : m;
+    } else {
+      const uint32_t w = qm::quantize_pack8(u, inv);
+      if (valid) cr[i] = w;
+    }
+    if (t + kQD < kQC) issue(d, j + kQD);
+  }
+}
+// Any parameter combination, one vector step at a time (loads not pipelined).
+template <int PASS>
+__device__ __forceinline__ void quant_step_generic(const uint4* __restrict__ xr, const float* __restrict__ bvec,
+                                                   const float* __restrict__ sa, float gamma, int had_block,
+                                                   float had_scale, int lane, int nv, int j, float inv,
+                                                   float& m, uint32_t* __restrict__ cr) {
+  const int i = lane + 32 * j;
+  const bool ok = i < nv;
+  const uint4 v = ok ? __ldg(xr + i) : make_uint4(0u, 0u, 0u, 0u);
+  float f[8], g[8], bb[8], u[8];
+  qm::unpack8(v, f);
+  if (had_block) qm::hadamard8(f, had_block, had_scale, lane);
+  qm::load_gb(sa, bvec, gamma, i, ok, g, bb);
+#pragma unroll
+  for (int e = 0; e < 8; ++e) u[e] = qm::affine(g[e], f[e], bb[e]);
+  if (ok) {
+    if (PASS == 0) m = qm::absmax8(m, u);
+    else cr[i] = qm::quantize_pack8(u, inv);
+  }
+}
+
 // ------------------------------------------------------------------------------ the kernel
 // ASYM (NEXT-1): unsigned activation codes, re-centred to q - 8 while they are expanded, and the
 // epilogue term (z_t + 8 s_t) s_w wsum[n].
@@ -227,7 +305,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
                  const GemmParams p) {
   using C = Cfg<FUSED>;
   constexpr int kEpiWarps = C::kEpiWarps;
-  constexpr int kSets = C::kSets;
+  constexpr int kEpiWarp0 = C::kEpiWarp0;
   constexpr int kAWarp0 = C::kAWarp0;
   constexpr int kUnpackWarp0 = C::kUnpackWarp0;
   constexpr int kProducerWarp = C::kProducerWarp, kProducerWarpB = C::kProducerWarpB, kMmaWarp = C::kMmaWarp;
@@ -235,14 +313,11 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
   // SWIZZLE_128B operands need 1024-byte alignment
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
-  // [ fused: int8 A stages | int8 B stages | packed ring | barriers ]
-  const uint32_t aop0 = smem_base;
-  uint8_t* aop_ptr = smem;
-  const uint32_t unpacked0 = smem_base + C::kAOperand;
+  // [ int8 B stages | packed ring | barriers | column operands | Y staging ]
+  const uint32_t unpacked0 = smem_base;
   const uint32_t packed0 = unpacked0 + kStages * C::kUnpackedStage;
-  uint8_t* unpacked_ptr = smem + C::kAOperand;
+  uint8_t* unpacked_ptr = smem;
   uint8_t* packed_ptr = unpacked_ptr + kStages * C::kUnpackedStage;
-  (void)aop0; (void)aop_ptr;
   Barriers* bars = reinterpret_cast<Barriers*>(packed_ptr + C::kPStages * C::kPackedStage);
 
   const int warp = threadIdx.x >> 5;
@@ -256,8 +331,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
   const uint4 hdr = ptx::ldg_nc(reinterpret_cast<const uint4*>(p.header));
 
   if (warp == kProducerWarp && lane == 0) {
-    if (!FUSED) ptx::prefetch_tensormap(&tmap_a);
-    if (C::kTmaStore) ptx::prefetch_tensormap(&tmap_y);
+    ptx::prefetch_tensormap(&tmap_a);
+    ptx::prefetch_tensormap(&tmap_y);
     for (int i = 0; i < C::kPStages; ++i) {
       ptx::mbar_init(ptx::smem_u32(&bars->pfull[i]), C::kPFullCount);
       ptx::mbar_init(ptx::smem_u32(&bars->pempty[i]), C::kPEmptyCount);
@@ -292,8 +367,25 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
   const int tile_step = static_cast<int>(gridDim.x) / CG;
   const int n_it = first_tile < num_tiles
                        ? ((num_tiles - first_tile + tile_step - 1) / tile_step) * p.num_kb : 0;
+  // tile -> (m_blk, n_blk).  Unfused: N-major walk (consecutive tiles share a weight strip).  Fused:
+  // M-major, so that a wave of tiles needs one or two 256-row strips of codes, in increasing order.
+  auto tile_m = [&](int tile) { return FUSED ? tile / p.num_n : tile % p.num_m; };
+  auto tile_n = [&](int tile) { return FUSED ? tile % p.num_n : tile / p.num_m; };
+  // fused: rows of this CTA's 128-row group of strip m that the quantiser warps will deliver
+  auto group_rows = [&](int m_blk) {
+    const int r0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM;
+    return r0 >= p.T ? 0 : (p.T - r0 < BM ? p.T - r0 : BM);
+  };
 
-  if ((warp == kProducerWarp && !FUSED) || warp == kProducerWarpB) {
+  // Fused variant: 1024 threads start with 64 registers each; the warpgroups trade them so that
+  // the epilogue warps get 80 and the quantiser group can hold a token row (up to kQV vectors per
+  // thread) in registers:
+  //   2 x 4 x 32 x 80 (epilogue) + 2 x 4 x 32 x 48 (A) + 2 x 4 x 32 x 40 (B) + 4 x 32 x 48 (roles)
+  //   + 4 x 32 x 128 (quantiser) = 65536.
+  if (warp >= C::kRoleWarp0 && warp < C::kRoleWarp0 + 4) {
+    if (FUSED) ptx::setmaxnreg_dec<48>();
+  }
+  if (warp == kProducerWarp || warp == kProducerWarpB) {
     // ===================================================================== producers (TMA)
     // Two warps, one per operand: a single warp's wait + expect_tx + two copy issues per k-block
     // is a ~350 clk serial chain (measured with everything else stubbed out).
@@ -301,10 +393,17 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     int stage = 0;
     uint32_t phase = 0;
     for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-      const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
+      const int m_blk = tile_m(tile), n_blk = tile_n(tile);
       const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM;
       // row groups of kTileRows rows: this CTA streams its half of the tile's N rows
       const uint8_t* g0 = p.tiles + static_cast<size_t>(2 * n_blk + rank) * p.num_kb * kTileBytes;
+      if (FUSED && is_a) {
+        // the codes of this CTA's 128 rows come from the quantiser warps of the whole grid
+        const unsigned int need = static_cast<unsigned int>(group_rows(m_blk));
+        const unsigned int* flag = p.ready + (2 * m_blk + static_cast<int>(rank));
+        while (ptx::ld_acquire_gpu(flag) < need) ptx::nanosleep(64);
+        ptx::fence_proxy_async_global();          // their generic-proxy stores -> this warp's TMA reads
+      }
       for (int kb = 0; kb < p.num_kb; ++kb) {
         ptx::mbar_wait(ptx::smem_u32(&bars->pempty[stage]), phase ^ 1u);
         const uint32_t full = ptx::smem_u32(&bars->pfull[stage]);
@@ -316,7 +415,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
             ptx::tma_load_2d(dst, &tmap_a, kb * (BK / 2), row0, full);
           } else {
             ptx::mbar_arrive_expect_tx(full, C::kPackedB);
-            ptx::bulk_load_1d(dst + C::kPackedAArea, g0 + static_cast<size_t>(kb) * kTileBytes,
+            ptx::bulk_load_1d(dst + kPackedA, g0 + static_cast<size_t>(kb) * kTileBytes,
                               kTileBytes, full);
           }
         }
@@ -335,8 +434,6 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       int as = 0;
       uint32_t phase = 0, aphase = 0;
       const uint64_t desc0 = ptx::make_smem_desc_sw128(unpacked0);
-      const uint64_t adesc0 = ptx::make_smem_desc_sw128(aop0);
-      (void)adesc0;
       // Flat k-block index over all of this CTA pair's tiles, unrolled over the kStages operand
       // stages: the stage index is a compile-time constant, so the barrier addresses, the TMEM
       // column of A and the descriptor of B are constants off loop-invariant bases (r1i capture:
@@ -361,12 +458,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
 #pragma unroll
               for (int k = 0; k < BK / 32; ++k) {
                 const uint32_t accum = (k != 0 || kb != 0) ? 1u : 0u;
-                if (FUSED) {
-                  const uint64_t da = adesc0 + static_cast<uint64_t>(stage * (kAStageBytes >> 4)) + 2 * k;
-                  ptx::mma_i8_ss_2cta(tmem_d, da, db + 2 * k, idesc, accum);
-                } else {
-                  ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
-                }
+                ptx::mma_i8_ts_2cta(tmem_d, a_col + k * 8, db + 2 * k, idesc, accum);
               }
               // frees the operand stage (A columns + B smem) in every CTA of the pair
               ptx::tcgen05_commit_2cta(ptx::smem_u32(&bars->empty[stage]), 3);
@@ -393,6 +485,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     }
   } else if (warp >= kUnpackWarp0 && warp < kUnpackWarp0 + kNumUnpackWarps * kSets) {
     // ===================================================================== B: int4 -> int8
+    if (FUSED) ptx::setmaxnreg_dec<40>();
     const int ut = (threadIdx.x - kUnpackWarp0 * 32) & 127;   // 0..127 inside the set
     const int set = (warp - kUnpackWarp0) >> 2;
     constexpr int kTasks = C::kBRows * 4 / (kNumUnpackWarps * 32);   // 16-byte chunks per thread
@@ -405,7 +498,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         const uint32_t ps = it % C::kPStages, us = it % kStages;      // unsigned: plain masks
         const uint32_t pphase = (it / C::kPStages) & 1u, uphase = (it / kStages) & 1u;
         ptx::mbar_wait(ptx::smem_u32(&bars->pfull[ps]), pphase);
-        const uint8_t* src = packed_ptr + ps * C::kPackedStage + C::kPackedAArea;
+        const uint8_t* src = packed_ptr + ps * C::kPackedStage + kPackedA;
         uint4 v[kTasks];
 #pragma unroll
         for (int i = 0; i < kTasks; ++i)
@@ -433,93 +526,65 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         }
       }
     }
-  } else if (FUSED && warp >= kAWarp0 && warp < kAWarp0 + 8) {
-    // ===================================================================== A: quantise in producer
-    // Eight warps x 32 lanes cover one 128-row x 128-channel k-block as 8 passes of 16 rows:
-    // lane = (row parity, vector v = lane & 15), so the 16 lanes of a half-warp hold the 128
-    // channels of one token (what the Hadamard's shuffle stages need) and a warp-wide load reads
-    // two rows x 256 contiguous bytes.  Same arithmetic (quant_math.cuh) and therefore the same
-    // codes as the stand-alone quantiser; the codes leave as 16 * q int8 in the even/odd order of
-    // the x16 expansion, straight into the SWIZZLE_128B operand stage.
-    const int aw = warp - kAWarp0;
-    const int v = lane & 15;
-    const int rbase = 2 * aw + (lane >> 4);               // rows rbase + 16 i, i = 0..7
-    const int r7 = rbase & 7;
-    const uint32_t full_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->full[0]), 0);
-    const uint32_t st_off = static_cast<uint32_t>((rbase >> 3) * 1024 + r7 * 128 + 4 * (v & 3));
-    const uint32_t ch_even = static_cast<uint32_t>(((2 * (v >> 2)) ^ r7) << 4);
-    const uint32_t ch_odd = static_cast<uint32_t>(((2 * (v >> 2) + 1) ^ r7) << 4);
-    // load cursor: one "half" (4 passes) ahead of the compute cursor
-    int l_tile = first_tile, l_kb = 0, l_half = 0;
-    auto load_half = [&](uint4 (&b)[4]) {
-      if (l_tile < num_tiles) {
-        const int row0 = (l_tile % p.num_m) * (BM * CG) + static_cast<int>(rank) * BM + rbase;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int row = row0 + 16 * (4 * l_half + i);
-          b[i] = row < p.T ? ptx::ldg_nc_stream(p.x + static_cast<int64_t>(row) * p.ldxv + l_kb * 16 + v)
-                           : make_uint4(0, 0, 0, 0);
-        }
-        if (++l_half == 2) {
-          l_half = 0;
-          if (++l_kb == p.num_kb) {
-            l_kb = 0;
-            l_tile += tile_step;
-          }
-        }
+  } else if (FUSED && warp < C::kQuantWarp0 + kQuantWarps) {
+    // ===================================================================== background quantiser
+    // One token row per warp (rows gw, gw + 4 * gridDim.x, ...: 256-row strips complete in the
+    // order the M-major tile walk needs them).  Lane l owns the 16-byte vectors l, l + 32, ... of
+    // the row, so an aligned half-warp holds 128 consecutive channels (what qm::hadamard8's shuffle
+    // stages expect; a 256-channel block spans the warp).  Same arithmetic (quant_math.cuh) and
+    // therefore the same codes as the stand-alone quantiser.  Two passes over the row -- absmax,
+    // then round and pack; the second one re-reads the row from L2 and recomputes u.  No
+    // shared-memory staging: the GEMM around these warps runs at the shared-memory bandwidth
+    // limit, and it leaves 40 % of the issue slots and most of HBM idle.
+    ptx::setmaxnreg_inc<128>();
+    const int gw = static_cast<int>(blockIdx.x) * kQuantWarps + (warp - C::kQuantWarp0);
+    const int gws = static_cast<int>(gridDim.x) * kQuantWarps;
+    const int nv = p.K >> 3;
+    const int nvl = (nv + 31) >> 5;                   // vectors per lane (the last one may be idle)
+    // 0 / 1: pipelined chunks without / with the block-128 Hadamard; 2: generic steps
+    const int mode = (p.bvec == nullptr || p.sa != nullptr) ? 2
+                     : p.had_block == 0 ? 0 : p.had_block == 128 ? 1 : 2;
+    for (int row = gw; row < p.T && num_tiles > 0; row += gws) {
+      const uint4* xr = p.x + static_cast<int64_t>(row) * p.ldxv;
+      uint32_t* cr = p.codes_out + static_cast<int64_t>(row) * nv;
+      float m = 0.0f;
+      if (mode == 0) {
+#pragma unroll 1
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<0, 0>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+      } else if (mode == 1) {
+#pragma unroll 1
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<0, 128>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+      } else {
+#pragma unroll 1
+        for (int j = 0; j < nvl; ++j)
+          quant_step_generic<0>(xr, p.bvec, p.sa, p.gamma, p.had_block, p.had_scale, lane, nv, j, 0.0f, m, cr);
       }
-    };
-    uint4 nxt[4];
-    load_half(nxt);
-    int us = 0;
-    uint32_t uphase = 0;
-    for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-      const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
-      const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM + rbase;
-      float inv[8];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int row = row0 + 16 * i;
-        inv[i] = row < p.T ? qm::reciprocal(p.scales[row]) : 0.0f;
+      for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+      const float st = qm::step_size(p.alpha, m);
+      const float inv = qm::reciprocal(st);
+      if (mode == 0) {
+#pragma unroll 1
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<1, 0>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+      } else if (mode == 1) {
+#pragma unroll 1
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<1, 128>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+      } else {
+#pragma unroll 1
+        for (int j = 0; j < nvl; ++j)
+          quant_step_generic<1>(xr, p.bvec, p.sa, p.gamma, p.had_block, p.had_scale, lane, nv, j, inv, m, cr);
       }
-      const bool dump = p.codes_dump != nullptr && n_blk == 0;
-      for (int kb = 0; kb < p.num_kb; ++kb) {
-        float g[8], bb[8];
-        qm::load_gb(p.sa, p.bvec, p.gamma, kb * 16 + v, true, g, bb);
-        ptx::mbar_wait(ptx::smem_u32(&bars->empty[us]), uphase ^ 1u);
-        uint8_t* stage = aop_ptr + us * kAStageBytes + st_off;
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          uint4 cur[4];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
-          load_half(nxt);
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            float f[8];
-            qm::unpack8(cur[i], f);
-            if (p.had_block) qm::hadamard8(f, p.had_block, p.had_scale, lane);
-            uint32_t t[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) t[e] = qm::code_bits(qm::affine(g[e], f[e], bb[e]), inv[4 * h + i]);
-            const uint32_t pn = qm::pack_nibbles(t);
-            uint8_t* dst = stage + (4 * h + i) * 2048;      // 16 rows = two 1024-byte swizzle atoms
-            *reinterpret_cast<uint32_t*>(dst + ch_even) = (pn << 4) & 0xF0F0F0F0u;
-            *reinterpret_cast<uint32_t*>(dst + ch_odd) = pn & 0xF0F0F0F0u;
-            if (dump) {
-              const int row = row0 + 16 * (4 * h + i);
-              if (row < p.T) p.codes_dump[static_cast<int64_t>(row) * (p.K / 8) + kb * 16 + v] = pn;
-            }
-          }
-        }
-        ptx::fence_proxy_async_smem();      // generic-proxy writes -> visible to tcgen05.mma
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_cluster(full_remote + us * 8);
-        advance(us, uphase, kStages);
-      }
+      if (lane == 0) p.scales_out[row] = st;
+      __syncwarp();
+      if (lane == 0) ptx::red_release_gpu_add(p.ready + (row >> 7), 1u);
     }
-  } else if (!FUSED && warp >= kAWarp0 && warp < kAWarp0 + 8) {
+  } else if (warp >= kAWarp0 && warp < kAWarp0 + 8) {
     // ===================================================================== A: smem -> TMEM
+    if (FUSED) ptx::setmaxnreg_dec<48>();
     // thread = token row = TMEM lane.  The packed tile is [128 rows][64 B] with TMA's SWIZZLE_64B
     // (16-byte chunk index ^= (row >> 1) & 3), so the 32 lanes' 16-byte reads of one chunk column
     // spread over all banks (4 wavefronts per 512 B: the minimum).
@@ -565,6 +630,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     }
   } else if (warp >= kEpiWarp0 && warp < kEpiWarp0 + kEpiWarps) {
     // ===================================================================== epilogue
+    if (FUSED) ptx::setmaxnreg_inc<80>();
     // 8 warps: warp % 4 = TMEM lane quarter (32 token rows), (warp - kEpiWarp0) / 4 = which half
     // of the tile's BN columns.  16 columns per tcgen05.ld keep the register footprint small.
     const int q = warp & 3;
@@ -581,7 +647,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     const int et = static_cast<int>(threadIdx.x) - kEpiWarp0 * 32;
     float pre[kPer][3];
     auto fetch = [&](int tile) {
-      const int nb = (tile / p.num_m) * BN;
+      const int nb = tile_n(tile) * BN;
 #pragma unroll
       for (int i = 0; i < kPer; ++i) {
         const int c = et + i * kEpiThreads;
@@ -593,7 +659,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       }
     };
     if (first_tile < num_tiles) fetch(first_tile);
-    // TMA-store epilogue (unfused): this warp's 32 x 96 bf16 block is staged in shared memory in the
+    // TMA-store epilogue: this warp's 32 x 96 bf16 block is staged in shared memory in the
     // SWIZZLE_64B layout of three 32-row x 64-byte boxes (lane = row, conflict-free STS.128) and
     // written by three bulk tensor stores -- a per-lane STG.128 touches 32 different 128-byte lines
     // (32 L1 tag cycles per instruction: 20 % of the LSU pipe's load in the r1h capture); TMA also
@@ -601,16 +667,26 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     const uint32_t stage_y = ptx::smem_u32(bars) + C::kTailBytes + (warp - kEpiWarp0) * C::kStoreWarpBytes;
     const uint32_t stage_lane = stage_y + lane * 64;
     const uint32_t stage_sw = (lane >> 1) & 3;
-    (void)stage_lane; (void)stage_sw;
     constexpr int kColsPerWarp = BN / (kEpiWarps / 4);
     const uint32_t tempty_remote = ptx::mapa_cluster(ptx::smem_u32(&bars->tempty[0]), 0);
     int as = 0;
     uint32_t aphase = 0;
     for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
-      const int m_blk = tile % p.num_m, n_blk = tile / p.num_m;
+      const int m_blk = tile_m(tile), n_blk = tile_n(tile);
       const int row = m_blk * (BM * CG) + static_cast<int>(rank) * BM + q * 32 + lane;
       const bool row_ok = row < p.T;
-      const float st = row_ok ? p.scales[row] : 0.0f;
+      float st = 0.0f;
+      if (FUSED) {
+        // the scale was written by a quantiser warp of some CTA during this launch: observe the
+        // group's counter (long complete: the A producer waited for it before this tile's first
+        // load) and read the scale past L1
+        const unsigned int need = static_cast<unsigned int>(group_rows(m_blk));
+        const unsigned int* flag = p.ready + (2 * m_blk + static_cast<int>(rank));
+        while (ptx::ld_acquire_gpu(flag) < need) ptx::nanosleep(64);
+        if (row_ok) st = ptx::ld_relaxed_gpu_f32(p.scales + row);
+      } else if (row_ok) {
+        st = p.scales[row];
+      }
       const float st256 = __fmul_rn(st, 0.00390625f);
       const float zt = (ASYM && row_ok) ? p.zeros[row] : 0.0f;
       const float midf = __fmaf_rn(8.0f, st, zt);
@@ -627,16 +703,13 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       ptx::bar_sync(1, kEpiThreads);
       if (tile + tile_step < num_tiles) fetch(tile + tile_step);
       cs += half * kColsPerWarp;
-      if (C::kTmaStore) {
-        if (lane == 0) ptx::bulk_wait_group_read<0>();   // the previous tile's stores have read the staging tile
-        __syncwarp();
-      }
+      if (lane == 0) ptx::bulk_wait_group_read<0>();   // the previous tile's stores have read the staging tile
+      __syncwarp();
       ptx::mbar_wait(ptx::smem_u32(&bars->tfull[as]), aphase);
       ptx::tcgen05_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + as * BN +
                              half * kColsPerWarp;
       const int n0 = n_blk * BN + half * kColsPerWarp;
-      uint16_t* yrow = p.y + static_cast<int64_t>(row) * p.ldy;
       // 8 columns: two groups of 4 -> one 16-byte store per row
       auto process8 = [&](const uint32_t (&r)[8], int c0) {
         uint32_t out[4];
@@ -677,13 +750,10 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
           out[(j >> 1) + 1] = lo23;
         }
         const int n = n0 + c0;
-        if (C::kTmaStore) {
-          const uint32_t dst = stage_lane + ((c0 >> 5) << 11) + ((((c0 >> 3) & 3) ^ stage_sw) << 4);
-          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(out[0]), "r"(out[1]),
-                       "r"(out[2]), "r"(out[3]) : "memory");
-        }
+        const uint32_t dst = stage_lane + ((c0 >> 5) << 11) + ((((c0 >> 3) & 3) ^ stage_sw) << 4);
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(out[0]), "r"(out[1]),
+                     "r"(out[2]), "r"(out[3]) : "memory");
         if (row_ok && n < p.N) {
-          if (!C::kTmaStore) *reinterpret_cast<uint4*>(yrow + n) = make_uint4(out[0], out[1], out[2], out[3]);
           if (p.acc_dump != nullptr) {
             int32_t* d = p.acc_dump + static_cast<int64_t>(row) * p.N + n;
 #pragma unroll
@@ -711,16 +781,14 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         process8(rb, c0 + 8);
       }
       ptx::tmem_ld_wait();
-      if (C::kTmaStore) {
-        ptx::fence_proxy_async_smem();                  // this lane's STS -> visible to the TMA engine
-        __syncwarp();
-        const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM + q * 32;
-        if (lane == 0 && row0 < p.T) {
+      ptx::fence_proxy_async_smem();                  // this lane's STS -> visible to the TMA engine
+      __syncwarp();
+      const int row0 = m_blk * (BM * CG) + static_cast<int>(rank) * BM + q * 32;
+      if (lane == 0 && row0 < p.T) {
 #pragma unroll
-          for (int bx = 0; bx < kColsPerWarp / 32; ++bx)
-            if (n0 + bx * 32 < p.N) ptx::tma_store_2d(&tmap_y, stage_y + bx * 2048, n0 + bx * 32, row0);
-          ptx::bulk_commit_group();
-        }
+        for (int bx = 0; bx < kColsPerWarp / 32; ++bx)
+          if (n0 + bx * 32 < p.N) ptx::tma_store_2d(&tmap_y, stage_y + bx * 2048, n0 + bx * 32, row0);
+        ptx::bulk_commit_group();
       }
       // all TMEM reads of this warp are complete (wait::ld above): release the accumulator
       ptx::tcgen05_fence_before();
@@ -731,7 +799,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
   }
 
   // ---- teardown: nobody leaves while the peer may still touch this CTA's barriers / smem
-  if (C::kTmaStore && warp >= kEpiWarp0 && warp < kEpiWarp0 + kEpiWarps && lane == 0)
+  if (warp >= kEpiWarp0 && warp < kEpiWarp0 + kEpiWarps && lane == 0)
     ptx::bulk_wait_group<0>();                          // Y stores complete before the CTA exits
   ptx::tcgen05_fence_before();
   __syncthreads();
@@ -747,6 +815,17 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
 
 // ------------------------------------------------------------------------------ host side
 namespace {
+
+// fused variant: [ ready counters, one per 128-row group, padded to 256 B | codes [T, K/2] ]
+struct FusedWorkspace {
+  size_t off_codes, bytes;
+};
+FusedWorkspace fused_workspace_layout(int T, int K) {
+  FusedWorkspace w{};
+  w.off_codes = (static_cast<size_t>((T + BM - 1) / BM) * 4 + 255) / 256 * 256;
+  w.bytes = w.off_codes + (static_cast<size_t>(T) * (K / 2) + 255) / 256 * 256;
+  return w;
+}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
@@ -862,21 +941,25 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
 
-  // A operand (unfused): codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows, SWIZZLE_64B;
+  // Fused variant: the workspace is [ ready counters | codes ]; the codes go to the caller's
+  // codes_dump instead when there is one (same layout, [T, K/2]).
+  const FusedWorkspace ws = fused_workspace_layout(g.T, g.K);
+  uint8_t* wsb = static_cast<uint8_t*>(g.workspace);
+  const uint8_t* codes = fused ? (g.codes_dump != nullptr ? g.codes_dump : wsb + ws.off_codes) : g.codes;
+
+  // A operand: codes [T, K/2] bytes; box = 64 bytes (128 int4) x 128 rows, SWIZZLE_64B;
   // rows beyond T are zero-filled by TMA, so a ragged last M tile needs no special case.
-  // Y (unfused): bf16 [T, ldy]; box = 32 columns (64 bytes) x 32 rows, SWIZZLE_64B; the store clips
+  // Y: bf16 [T, ldy]; box = 32 columns (64 bytes) x 32 rows, SWIZZLE_64B; the store clips
   // rows >= T and columns >= N.
   CUtensorMap tmap_a{}, tmap_y{};
-  if (!fused) {
-    cudaError_t e = tensor_map_2d(g.codes, static_cast<uint64_t>(g.K / 2), static_cast<uint64_t>(g.T),
-                                  static_cast<uint64_t>(g.K / 2), BK / 2, BM, CU_TENSOR_MAP_DATA_TYPE_UINT8,
-                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, &tmap_a);
-    if (e != cudaSuccess) return e;
-    e = tensor_map_2d(g.y, static_cast<uint64_t>(g.N), static_cast<uint64_t>(g.T),
-                      static_cast<uint64_t>(g.ldy) * 2, 32, 32, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
-                      CU_TENSOR_MAP_L2_PROMOTION_NONE, &tmap_y);
-    if (e != cudaSuccess) return e;
-  }
+  cudaError_t e = tensor_map_2d(codes, static_cast<uint64_t>(g.K / 2), static_cast<uint64_t>(g.T),
+                                static_cast<uint64_t>(g.K / 2), BK / 2, BM, CU_TENSOR_MAP_DATA_TYPE_UINT8,
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, &tmap_a);
+  if (e != cudaSuccess) return e;
+  e = tensor_map_2d(g.y, static_cast<uint64_t>(g.N), static_cast<uint64_t>(g.T),
+                    static_cast<uint64_t>(g.ldy) * 2, 32, 32, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, &tmap_y);
+  if (e != cudaSuccess) return e;
 
   GemmParams p{};
   p.header = reinterpret_cast<const uint32_t*>(base);
@@ -899,12 +982,18 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   if (fused) {
     p.x = static_cast<const uint4*>(g.x);
     p.ldxv = g.ldx / 8;
+    p.alpha = g.alpha;
     p.gamma = g.gamma;
     p.sa = g.sa;
     p.bvec = g.b;
     p.had_block = g.had_block;
     p.had_scale = g.had_scale;
-    p.codes_dump = reinterpret_cast<uint32_t*>(g.codes_dump);
+    p.codes_out = reinterpret_cast<uint32_t*>(const_cast<uint8_t*>(codes));
+    p.scales_out = const_cast<float*>(g.scales);
+    p.ready = reinterpret_cast<unsigned int*>(wsb);
+    // the counters start at zero (the workspace keeps whatever the last call left)
+    e = cudaMemsetAsync(wsb, 0, ws.off_codes, g.stream);
+    if (e != cudaSuccess) return e;
     return launch_pair<true, false>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
   }
   if (g.zeros != nullptr) return launch_pair<false, true>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
@@ -913,35 +1002,12 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
 
 // ------------------------------------------------------------------------------ fused variant (a10)
 size_t fused_workspace_bytes(int T, int N, int K) {
-  (void)T; (void)N; (void)K;
-  return 256;   // the quantise-in-producer kernel keeps everything on chip
+  (void)N;
+  return fused_workspace_layout(T, K).bytes;
 }
 
-bool fused_supported(int had_block) { return had_block <= 128; }   // 16 lanes hold 128 channels
+bool fused_supported(int had_block) { return had_block <= 256; }   // a block spans at most one warp
 
-cudaError_t launch_linear_fused(const GemmLaunch& g) {
-  // pass 1: per-token absmax -> scales (reads X once, writes T floats)
-  QuantLaunch q{};
-  q.x = g.x;
-  q.ldx = g.ldx;
-  q.T = g.T;
-  q.K = g.K;
-  q.alpha = g.alpha;
-  q.gamma = g.gamma;
-  q.sa = g.sa;
-  q.b = g.b;
-  q.had_block = g.had_block;
-  q.had_scale = g.had_scale;
-  q.codes = nullptr;
-  q.scales = const_cast<float*>(g.scales);
-  q.stream = g.stream;
-  q.num_sms = g.num_sms;
-  q.device = g.device;
-  q.blocks_per_sm = 2;
-  const cudaError_t e = launch_quantize_act(q, false);
-  if (e != cudaSuccess) return e;
-  // pass 2: GEMM with the quantise-in-producer warps
-  return launch_w4a4_gemm(g);
-}
+cudaError_t launch_linear_fused(const GemmLaunch& g) { return launch_w4a4_gemm(g); }
 
 }  // namespace baseq

@@ -381,14 +381,38 @@ def test_fused_per_channel_sa_and_no_bias():
     run_fused(x, _rand_w(rng, N, K, bias=False), 1.0, 1.0, None, sa=sa)
 
 
-def test_fused_rejects_hadamard_256():
-    x = torch.zeros((4, 512), dtype=torch.bfloat16, device="cuda")
-    rng = np.random.default_rng(1)
-    W = _rand_w(rng, 8, 512)
-    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]))
-    with pytest.raises(bq.BaseqError) as e:
-        bq.linear_fused(x, bq.ActParams(0.9, had_block=256), pw)
-    assert e.value.status == 6
+def test_fused_hadamard_256_and_many_rows_per_quantiser_warp():
+    # a 256-channel block spans the whole quantiser warp; few tiles = few CTAs = many rows per warp
+    rng = np.random.default_rng(256)
+    T, K, N = 700, 1024, 136
+    x = rand_x(rng, T, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    run_fused(x, _rand_w(rng, N, K), 0.9, 1.05, b, had_block=256)
+    T, K, N = 1500, 640, 72                     # K / 8 = 80 vectors: a ragged last step per lane
+    x = rand_x(rng, T, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    run_fused(x, _rand_w(rng, N, K), 1.0, 1.0, b, had_block=128)
+
+
+def test_fused_workspace_is_reused_without_clearing():
+    # the ready counters are reset by the call itself: same workspace, garbage in it, three calls
+    rng = np.random.default_rng(77)
+    T, K, N = 300, 512, 200
+    x_bits = rand_x(rng, T, K)
+    W = _rand_w(rng, N, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(b), dev(W["layer_bias"]))
+    params = bq.ActParams(0.9, 1.05, None, dev(b), 0)
+    ref = oracle.linear(x_bits, W["w_nibbles"], W["w_scale"], fb, 0.9, 1.05, None, b, 0)
+    ws = torch.full((bq.lib().baseq_fused_workspace_bytes(T, N, K),), 0xFF, dtype=torch.uint8, device="cuda")
+    x = bf16_dev(x_bits)
+    for _ in range(3):
+        y, scales = bq.linear_fused(x, params, pw, workspace=ws)
+        assert np.array_equal(bits_host(y), ref["y"])
+        assert np.array_equal(scales.cpu().numpy().view(np.uint32), ref["scales"].view(np.uint32))
+    off = ws.numel() - T * K // 2                                     # [ counters | codes ]
+    assert np.array_equal(ws[off:].cpu().numpy().reshape(T, K // 2), ref["codes"])
 
 
 # ------------------------------------------------------------------------------- full BASELINE sizes
