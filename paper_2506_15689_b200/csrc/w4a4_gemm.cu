@@ -159,29 +159,30 @@ __device__ __forceinline__ void advance(int& stage, uint32_t& phase, int n) {
 //
 //   t   = RN(s_t * acc)            rel. error <= 2^-24
 //   y   = RN(t * s_w + fb)         one more rounding
-//   |y - y*| <= 2^-24 (|t s_w| + |y|) (1 + eps)  <  E := 2^-23 (|RN(t s_w)| + |y|)
-// If bf16(y - E) == bf16(y + E) every real number in the bracket -- including the fp64 value --
-// rounds to that bf16.
-// One output.  Fast path: t = RN(s_t * accf), p = RN(t * s_w), y = RN(t * s_w + fb) and the
-// bracket [y - E, y + E] with E = 2^-23 (|p| + |y|) >= 2 |y - y*| (see above); when both ends round
-// to the same bf16 (all but ~2.4e-4 of the elements, whatever the cancellation between p and fb)
-// that is the result, otherwise the fp64 expression itself is evaluated.
+// If bf16(y - E) == bf16(y + E) for a proven bound E >= |y - y*| every real number in the bracket
+// -- including the fp64 value -- rounds to that bf16 (all but ~2.4e-4 of the elements); otherwise
+// the fp64 expression itself is evaluated.  The bound is derived at dequant_bracket below.
 __device__ __noinline__ uint32_t dequant_f64(int32_t acc, float st, float sw, float fb) {
   return epi::dequant_f64(acc, st, sw, fb);
 }
 // `raw` is the TMEM accumulator 256 * acc (|acc| < 2^22, so raw has at most 22 significant bits
 // and converts to fp32 exactly) and st256 = s_t * 2^-8 (exact): st256 * float(raw) is the same
 // real number as s_t * acc and rounds to the same t.
-// Branch-free fast path: returns the packed pair (bf16(hi) << 16) | bf16(lo) of the bracket ends
-//   hi, lo = y +- 2^-23 (|p| + |y| + 2^-100)
-// (the 2^-100 keeps the bracket wider than the absolute rounding errors when y is denormal).
-// The element is settled iff both halves are equal.
-__device__ __forceinline__ void dequant_bracket(int32_t raw, float st256, float sw, float fb,
+// Branch-free fast path: returns the bracket ends  hi, lo = y +- 2^-23 (2 |y| + |fb| + 2^-100)
+// (the 2^-100 keeps the bracket wider than the absolute rounding errors when y is denormal; the
+// caller passes fbt = |fb| + 2^-100, formed once per column when the tile's operands are staged).
+// With P = s_t s_w acc:  y = (P (1 + d1) + fb)(1 + d2), |d| <= 2^-24, so
+//   |y - y*| <= 2^-24 (|P| + |y|)(1 + 2^-23)  and  |P| = |y* - fb| <= |y| + |y - y*| + |fb|,
+// i.e. |y - y*| < 2^-24 (2 |y| + |fb|)(1 + 2^-22): E is twice that, which also covers the rounding of
+// hi / lo themselves (half an ulp of y).  Five fma-pipe instructions per output (t, y, s, hi, lo)
+// instead of seven: the epilogue's FMUL / FFMA / FADD are what a tile costs the main loop
+// (r1i capture: ~2400 clk per tile, the fma pipe issues one warp instruction per two clocks).
+// The element is settled iff both ends round to the same bf16.
+__device__ __forceinline__ void dequant_bracket(int32_t raw, float st256, float sw, float fb, float fbt,
                                                 float& lo, float& hi) {
   const float t = __fmul_rn(st256, __int2float_rn(raw));
-  const float p = __fmul_rn(t, sw);
   const float y = __fmaf_rn(t, sw, fb);
-  const float s = __fadd_rn(__fadd_rn(fabsf(p), 7.888609052210118e-31f), fabsf(y));
+  const float s = __fmaf_rn(2.0f, fabsf(y), fbt);
   hi = __fmaf_rn(s, 1.1920928955078125e-07f, y);
   lo = __fmaf_rn(s, -1.1920928955078125e-07f, y);
 }
@@ -697,7 +698,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         if (c < BN) {
           cs[c] = pre[i][0];
           cs[BN + c] = pre[i][1];
-          if (ASYM) cs[2 * BN + c] = pre[i][2];
+          // third column operand: wsum (asymmetric) or |fb| + 2^-100 for the bracket
+          cs[2 * BN + c] = ASYM ? pre[i][2] : __fadd_rn(fabsf(pre[i][1]), 7.888609052210118e-31f);
         }
       }
       ptx::bar_sync(1, kEpiThreads);
@@ -717,15 +719,14 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         for (int j = 0; j < 8; j += 4) {
           const float4 sw = *reinterpret_cast<const float4*>(cs + c0 + j);
           const float4 fb = *reinterpret_cast<const float4*>(cs + BN + c0 + j);
-          float4 ws = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-          if (ASYM) ws = *reinterpret_cast<const float4*>(cs + 2 * BN + c0 + j);
+          const float4 ws = *reinterpret_cast<const float4*>(cs + 2 * BN + c0 + j);
           const float swv[4] = {sw.x, sw.y, sw.z, sw.w}, fbv[4] = {fb.x, fb.y, fb.z, fb.w};
           const float wsv[4] = {ws.x, ws.y, ws.z, ws.w};
           float lo[4], hi[4];
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             if (ASYM) dequant_bracket_asym(static_cast<int32_t>(r[j + e]), st256, midf, swv[e], fbv[e], wsv[e], lo[e], hi[e]);
-            else dequant_bracket(static_cast<int32_t>(r[j + e]), st256, swv[e], fbv[e], lo[e], hi[e]);
+            else dequant_bracket(static_cast<int32_t>(r[j + e]), st256, swv[e], fbv[e], wsv[e], lo[e], hi[e]);
           }
           // output words of the low ends and of the high ends of the four brackets
           uint32_t lo01 = pack_bf16x2(lo[1], lo[0]), lo23 = pack_bf16x2(lo[3], lo[2]);
