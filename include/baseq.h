@@ -200,10 +200,13 @@ BASEQ_API baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int 
  * the same contract and the same bits as baseq_quantize_act followed by baseq_w4a4_gemm.
  * had_block: 0 or any power of two <= 256 dividing K (128 and 0 at full speed).
  *   workspace / workspace_bytes  device scratch of at least baseq_fused_workspace_bytes(T, N, K)
- *                = 256-byte-rounded counters + T * K / 2 bytes, 256-byte aligned; its contents on
- *                entry do not matter (the call clears its counters on the stream first), it may
- *                be reused by the next call on the same stream, and two calls that overlap on the
- *                GPU must not share it
+ *                = a 256-byte control block + 256-byte-rounded counters + T * K / 2 bytes,
+ *                256-byte aligned.  Its contents on entry do not matter: the kernel clears its own
+ *                counters and announces that through a 64-bit word of the control block, which its
+ *                last CTA resets (memory that was never a workspace carries that word by chance
+ *                with probability 2^-64); nothing but the kernel is enqueued, so the call can be
+ *                captured in a CUDA graph and replayed.  It may be reused by the next call on the
+ *                same stream; two calls that overlap on the GPU must not share it
  *   codes_dump   optional [T, K/2]: the codes are written there instead of the workspace, or NULL
  *   scales_out   [T] required                                                                */
 BASEQ_API size_t baseq_fused_workspace_bytes(int T, int N, int K);

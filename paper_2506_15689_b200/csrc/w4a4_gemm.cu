@@ -141,7 +141,10 @@ struct GemmParams {
   float had_scale;
   uint32_t* codes_out;      // [T, K/8] words of 8 nibbles: the workspace (or the caller's codes_dump)
   float* scales_out;        // [T] (= scales)
-  unsigned int* ready;      // [ceil(T / 128)] rows quantised per 128-row group, zero at launch
+  unsigned int* ready;      // [ceil(T / 128)] rows quantised per 128-row group
+  unsigned long long* ctrl; // workspace control block: [0] = kFusedReady once the counters are zero,
+                            // [1] (low word) = CTAs that have finished
+  int ngroups;
 };
 
 __device__ __forceinline__ void advance(int& stage, uint32_t& phase, int n) {
@@ -297,6 +300,18 @@ __device__ __forceinline__ void quant_step_generic(const uint4* __restrict__ xr,
   }
 }
 
+// Fused variant: the workspace's counters start from whatever the last user of the memory left.
+// CTA 0 clears them (and the CTA-exit count) and then publishes kFusedReady in the control block;
+// every reader or incrementer of a counter first waits for that word; the last CTA to finish puts
+// the word back to 0, so the next call on this workspace -- or the next replay of a captured graph
+// -- finds it unset again.  (A memset node in front of the kernel would do, but it serialises the
+// launch against its predecessor: ~6 us per call.)  Memory that has never been a workspace holds
+// the 64-bit word by chance with probability 2^-64.
+constexpr unsigned long long kFusedReady = 0x51534142465553EDull;
+__device__ __forceinline__ void fused_wait_ready(const unsigned long long* ctrl) {
+  while (ptx::ld_acquire_gpu_u64(ctrl) != kFusedReady) ptx::nanosleep(64);
+}
+
 // ------------------------------------------------------------------------------ the kernel
 // ASYM (NEXT-1): unsigned activation codes, re-centred to q - 8 while they are expanded, and the
 // epilogue term (z_t + 8 s_t) s_w wsum[n].
@@ -402,6 +417,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         // the codes of this CTA's 128 rows come from the quantiser warps of the whole grid
         const unsigned int need = static_cast<unsigned int>(group_rows(m_blk));
         const unsigned int* flag = p.ready + (2 * m_blk + static_cast<int>(rank));
+        if (tile == first_tile) fused_wait_ready(p.ctrl);
         while (ptx::ld_acquire_gpu(flag) < need) ptx::nanosleep(64);
         ptx::fence_proxy_async_global();          // their generic-proxy stores -> this warp's TMA reads
       }
@@ -545,6 +561,17 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     // 0 / 1: pipelined chunks without / with the block-128 Hadamard; 2: generic steps
     const int mode = (p.bvec == nullptr || p.sa != nullptr) ? 2
                      : p.had_block == 0 ? 0 : p.had_block == 128 ? 1 : 2;
+    if (gw == 0 && num_tiles > 0) {
+      // clear the counters and the exit count, then publish: see kFusedReady
+      for (int i = lane; i < p.ngroups; i += 32) p.ready[i] = 0u;
+      if (lane == 0) p.ctrl[1] = 0ull;
+      __syncwarp();
+      if (lane == 0) {
+        __threadfence();
+        ptx::st_release_gpu_u64(p.ctrl, kFusedReady);
+      }
+    }
+    bool seen_ready = false;
     for (int row = gw; row < p.T && num_tiles > 0; row += gws) {
       const uint4* xr = p.x + static_cast<int64_t>(row) * p.ldxv;
       uint32_t* cr = p.codes_out + static_cast<int64_t>(row) * nv;
@@ -581,7 +608,11 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       }
       if (lane == 0) p.scales_out[row] = st;
       __syncwarp();
-      if (lane == 0) ptx::red_release_gpu_add(p.ready + (row >> 7), 1u);
+      if (lane == 0) {
+        if (!seen_ready) fused_wait_ready(p.ctrl);
+        ptx::red_release_gpu_add(p.ready + (row >> 7), 1u);
+      }
+      seen_ready = true;
     }
   } else if (warp >= kAWarp0 && warp < kAWarp0 + 8) {
     // ===================================================================== A: smem -> TMEM
@@ -683,6 +714,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         // load) and read the scale past L1
         const unsigned int need = static_cast<unsigned int>(group_rows(m_blk));
         const unsigned int* flag = p.ready + (2 * m_blk + static_cast<int>(rank));
+        if (tile == first_tile) fused_wait_ready(p.ctrl);
         while (ptx::ld_acquire_gpu(flag) < need) ptx::nanosleep(64);
         if (row_ok) st = ptx::ld_relaxed_gpu_f32(p.scales + row);
       } else if (row_ok) {
@@ -804,6 +836,11 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     ptx::bulk_wait_group<0>();                          // Y stores complete before the CTA exits
   ptx::tcgen05_fence_before();
   __syncthreads();
+  if (FUSED && num_tiles > 0 && threadIdx.x == 0) {
+    // every role of this CTA is past its last look at the control word: count the exit
+    const unsigned int done = atomicAdd(reinterpret_cast<unsigned int*>(p.ctrl + 1), 1u);
+    if (done == gridDim.x - 1) ptx::st_release_gpu_u64(p.ctrl, 0ull);
+  }
   ptx::cluster_sync_all();
   if (warp == kMmaWarp) {
     ptx::tcgen05_fence_after();
@@ -817,13 +854,17 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
 // ------------------------------------------------------------------------------ host side
 namespace {
 
-// fused variant: [ ready counters, one per 128-row group, padded to 256 B | codes [T, K/2] ]
+// fused variant: [ control block 256 B | ready counters, one per 128-row group, padded to 256 B |
+// codes [T, K/2] ]
 struct FusedWorkspace {
-  size_t off_codes, bytes;
+  size_t off_ready, off_codes, bytes;
+  int ngroups;
 };
 FusedWorkspace fused_workspace_layout(int T, int K) {
   FusedWorkspace w{};
-  w.off_codes = (static_cast<size_t>((T + BM - 1) / BM) * 4 + 255) / 256 * 256;
+  w.ngroups = (T + BM - 1) / BM;
+  w.off_ready = 256;
+  w.off_codes = w.off_ready + (static_cast<size_t>(w.ngroups) * 4 + 255) / 256 * 256;
   w.bytes = w.off_codes + (static_cast<size_t>(T) * (K / 2) + 255) / 256 * 256;
   return w;
 }
@@ -942,8 +983,8 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
 
-  // Fused variant: the workspace is [ ready counters | codes ]; the codes go to the caller's
-  // codes_dump instead when there is one (same layout, [T, K/2]).
+  // Fused variant: the workspace is [ control block | ready counters | codes ]; the codes go to the
+  // caller's codes_dump instead when there is one (same layout, [T, K/2]).
   const FusedWorkspace ws = fused_workspace_layout(g.T, g.K);
   uint8_t* wsb = static_cast<uint8_t*>(g.workspace);
   const uint8_t* codes = fused ? (g.codes_dump != nullptr ? g.codes_dump : wsb + ws.off_codes) : g.codes;
@@ -991,10 +1032,9 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
     p.had_scale = g.had_scale;
     p.codes_out = reinterpret_cast<uint32_t*>(const_cast<uint8_t*>(codes));
     p.scales_out = const_cast<float*>(g.scales);
-    p.ready = reinterpret_cast<unsigned int*>(wsb);
-    // the counters start at zero (the workspace keeps whatever the last call left)
-    e = cudaMemsetAsync(wsb, 0, ws.off_codes, g.stream);
-    if (e != cudaSuccess) return e;
+    p.ctrl = reinterpret_cast<unsigned long long*>(wsb);
+    p.ready = reinterpret_cast<unsigned int*>(wsb + ws.off_ready);
+    p.ngroups = ws.ngroups;
     return launch_pair<true, false>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
   }
   if (g.zeros != nullptr) return launch_pair<false, true>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);

@@ -55,8 +55,8 @@ def test_size_queries_and_blob_layout():
         npad = -(-N // 192) * 192                               # tile N extent
         assert nb == 128 + 12 * npad + npad * K // 2
     assert L.baseq_fused_workspace_bytes(0, 8, 128) == 0
-    assert L.baseq_fused_workspace_bytes(16, 256, 256) == 256 + 16 * 128     # counters + codes [T, K/2]
-    assert L.baseq_fused_workspace_bytes(4096, 8192, 28672) == 256 + 4096 * 14336
+    assert L.baseq_fused_workspace_bytes(16, 256, 256) == 512 + 16 * 128     # control + counters + codes [T, K/2]
+    assert L.baseq_fused_workspace_bytes(4096, 8192, 28672) == 512 + 4096 * 14336
     assert L.baseq_linear_host_scratch_bytes(16, 256, 256) >= 16 * 256 * 2 + 16 * 128 + 64 + 16 * 256 * 2
 
 
@@ -88,7 +88,7 @@ def test_validation_happens_before_any_launch():
     # the fused and the host-buffer entry points run every check of BOTH stages before the first
     # launch or copy (a failing call enqueues nothing): these all fail before the device is queried
     assert f(base, 256, 4, 256, ctypes.byref(ok), base, 8, base, 8, base, 512, None, base, None,
-             None) == 5                                   # workspace = ready counters (256) + codes (512)
+             None) == 5                                   # workspace = control 256 + counters 256 + codes 512
     bad_alpha = P(0.0, 1.0, None, None, 0)
     assert f(base, 256, 4, 256, ctypes.byref(bad_alpha), base, 8, base, 8, base, 4096, None, base, None,
              None) == 4
