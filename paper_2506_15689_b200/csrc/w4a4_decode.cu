@@ -3,10 +3,12 @@
 // work is streaming the packed weights once (N K / 2 bytes) and the 128 x 192 tcgen05 tile would
 // be 1-50 % full.  HBM-bound: algorithmic bytes = N K / 2 (W) + T K / 2 (codes) + 2 T N (Y).
 //
-//   CTA            MT groups of 16 output channels (MT = 2 for T > 16 and N >= 64 SMs, else 1; a group is 16 rows x
+//   CTA            MT groups of 16 output channels (MT = 2 for T > 16 and N >= 64 SMs, for T <= 8 and
+//                  N >= 48 SMs, else 1; a group is 16 rows x
 //                  64 bytes = 1 KB contiguous per k-block of the weight blob), all of K, all T
 //                  tokens; grid = ceil(N / (16 MT))
-//   8 warps        k-blocks w, w + 8, ... each, through a rolling window of kDepth register slots
+//   8 warps        k-blocks w, w + 8, ... each, through a window of kDepth register slots (T <= 16:
+//                  branch-free straight-line pieces, see the main loop; T > 16: a rolling window)
 //                  (2 MT x LDG.128 per lane and k-block, streaming; the first window is issued
 //                  BEFORE griddepcontrol.wait: the weights do not depend on the preceding
 //                  quantiser, and griddepcontrol.launch_dependents right after it lets a following
@@ -327,9 +329,13 @@ cudaError_t launch_nt(const DecodeParams& p, cudaStream_t stream) {
 // costs more than the sharing saves there, and less at T = 64).
 template <bool ASYM>
 cudaError_t launch_asym(const DecodeParams& p, int num_sms, cudaStream_t stream) {
+  const bool wide = p.N >= 2 * kRows * 2 * num_sms;
+  // T <= 8: two groups per CTA (64 KB per CTA and k-sweep, half as many CTAs) where that still
+  // leaves 1.5 CTAs per SM (measured with the straight-line pieces: c3 17.9 -> 15.7 us, c5 24.4 ->
+  // 21.3 us at T = 1; at N = 4096 the 128-CTA grid loses, and T = 16 does not gain)
+  if (p.T <= 8 && p.N >= 48 * num_sms) return launch_nt<1, 2, ASYM>(p, stream);
   if (p.T <= 8) return launch_nt<1, 1, ASYM>(p, stream);
   if (p.T <= 16) return launch_nt<2, 1, ASYM>(p, stream);
-  const bool wide = p.N >= 2 * kRows * 2 * num_sms;
   if (p.T <= 32) return wide ? launch_nt<4, 2, ASYM>(p, stream) : launch_nt<4, 1, ASYM>(p, stream);
   return launch_nt<8, 2, ASYM>(p, stream);
 }

@@ -878,6 +878,22 @@ def test_decode_k_and_n_edges(T, K, N):
     run_asym(x, W, 1.0, 1.0, b)
 
 
+@pytest.mark.parametrize("T,K,N", [(8, 28672, 64), (3, 6144, 72), (16, 6144, 40), (8, 8192, 7112),
+                                   (5, 512, 7120), (2, 1280, 7104), (6, 3072, 7104), (1, 11008, 7104)])
+def test_decode_straight_line_pieces(T, K, N):
+    # T <= 16 walks a warp's k-blocks in branch-free pieces (w4a4_decode.cu): every piece kind --
+    # several full pieces + an exact short one (K = 28672: 28 k-blocks per warp), a masked full piece
+    # (K = 6144: 6), a masked short one, warps without any k-block (K = 512) -- and, for T <= 8 and
+    # N >= 48 x 148, the two-groups-per-CTA instantiation (window of 2: full + full, exact short,
+    # masked full at K = 3072, full + masked at K = 11008), N % 32 != 0 included
+    rng = np.random.default_rng(7 * T + 3 * K + 11 * N)
+    x = rand_x(rng, T, K, spread=1.0)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    W = _rand_w(rng, N, K)
+    run_linear(x, W, 0.9, 1.0, b)
+    run_asym(x, W, 1.0, 1.0, b)
+
+
 def test_decode_extreme_codes():
     # largest raw accumulators: qa = -8, qw = -8 -> acc = 64 K; qa = 7, qw = -8 -> -56 K (closed forms)
     T, K, N = 48, 28672, 64
