@@ -236,11 +236,18 @@ __device__ __forceinline__ void dequant_bracket_asym(int32_t raw, float st256, f
 // values} is a true software pipeline.  HAD: 0 = no rotation, 128 = block-128 Hadamard (compile
 // time: qm::hadamard8 unrolls to 32 shuffles); everything else takes the generic step below.
 constexpr int kQD = 4;     // ring slots = loads in flight per lane: x + 2 x b per slot
-constexpr int kQC = 8;     // vector steps per chunk
-template <int PASS, int HAD>
+constexpr int kQC = 8;     // vector steps per chunk (16 without the Hadamard measured 4 % slower for
+                           // the whole launch on K = 4096: twice the code in the instruction cache)
+constexpr int kQCLong = kQC;
+// GBF16 (HAD == 0 only): the scalar s^a is a bf16 value, so Q0 + Q2 are ONE mixed-precision fma per
+// element (as in the stand-alone quantiser, quant_math.cuh) -- computed as -u = fma(x, -gamma, b),
+// which needs no negated copy of b; |-u| = |u| for the absmax, and pass 1 rounds (-u) * (-inv), the
+// same exact product as u * inv.
+template <int PASS, int HAD, bool GBF16, int QC>
 __device__ __forceinline__ void quant_chunk(const uint4* __restrict__ xr, const float* __restrict__ bvec,
                                             float gamma, float had_scale, int lane, int nv, int nvl,
                                             int c0, float inv, float& m, uint32_t* __restrict__ cr) {
+  static_assert(!(GBF16 && HAD != 0), "the bf16 fma consumes the packed activations as they are");
   uint4 sx[kQD];
   float4 sb0[kQD], sb1[kQD];
   auto issue = [&](int d, int j) {
@@ -254,29 +261,37 @@ __device__ __forceinline__ void quant_chunk(const uint4* __restrict__ xr, const 
   for (int d = 0; d < kQD; ++d) issue(d, c0 + d);
   if (PASS == 0) {
     // the chunk after the next one, towards L2: the ring's own depth covers an L2 hit, not an HBM miss
-    const int jp = c0 + 2 * kQC + (lane >> 2);            // 8 steps x 4 lines of 128 bytes
-    if (jp < nvl) ptx::prefetch_l2(reinterpret_cast<const uint8_t*>(xr + 32 * jp) + 128 * (lane & 3));
+    // (measured: asking for the next row's head during pass 1 as well cost 4 % of the fused launch)
+    const int jp = c0 + 2 * QC + (lane >> 2);             // 8 steps x 4 lines of 128 bytes
+    const int vp = 32 * jp + 8 * (lane & 3);              // first vector of this lane's line
+    if (vp < nv) ptx::prefetch_l2(xr + vp);               // never past the end of the row
   }
 #pragma unroll
-  for (int t = 0; t < kQC; ++t) {
+  for (int t = 0; t < QC; ++t) {
     const int d = t % kQD;
     const int j = c0 + t;
     const int i = lane + 32 * j;
     const bool valid = j < nvl && i < nv;
-    float f[8], u[8];
-    qm::unpack8(sx[d], f);
-    if (HAD != 0) qm::hadamard8(f, HAD, had_scale, lane);
+    float u[8];
     const float bb[8] = {sb0[d].x, sb0[d].y, sb0[d].z, sb0[d].w, sb1[d].x, sb1[d].y, sb1[d].z, sb1[d].w};
+    if (GBF16) {
+      const uint32_t ng = (__float_as_uint(gamma) >> 16) ^ 0x8000u;       // -gamma as bf16 bits
+      qm::affine8_bf16(sx[d], ng, bb, u);                                 // u := -(gamma x - b)
+    } else {
+      float f[8];
+      qm::unpack8(sx[d], f);
+      if (HAD != 0) qm::hadamard8(f, HAD, had_scale, lane);
 #pragma unroll
-    for (int e = 0; e < 8; ++e) u[e] = qm::affine(gamma, f[e], bb[e]);
+      for (int e = 0; e < 8; ++e) u[e] = qm::affine(gamma, f[e], bb[e]);
+    }
     if (PASS == 0) {
       const float mm = qm::absmax8(m, u);
       m = valid ? mm : m;
     } else {
-      const uint32_t w = qm::quantize_pack8(u, inv);
+      const uint32_t w = qm::quantize_pack8(u, GBF16 ? -inv : inv);
       if (valid) cr[i] = w;
     }
-    if (t + kQD < kQC) issue(d, j + kQD);
+    if (t + kQD < QC) issue(d, j + kQD);
   }
 }
 // Any parameter combination, one vector step at a time (loads not pipelined).
@@ -558,9 +573,11 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     const int gws = static_cast<int>(gridDim.x) * kQuantWarps;
     const int nv = p.K >> 3;
     const int nvl = (nv + 31) >> 5;                   // vectors per lane (the last one may be idle)
-    // 0 / 1: pipelined chunks without / with the block-128 Hadamard; 2: generic steps
+    // 0 / 1: pipelined chunks without / with the block-128 Hadamard; 3: as 0 with the bf16 fma
+    // (scalar s^a that is a bf16 value: 1.0 in four of the five configs); 2: generic steps
     const int mode = (p.bvec == nullptr || p.sa != nullptr) ? 2
-                     : p.had_block == 0 ? 0 : p.had_block == 128 ? 1 : 2;
+                     : p.had_block == 0 ? (qm::is_bf16_value(p.gamma) ? 3 : 0)
+                     : p.had_block == 128 ? 1 : 2;
     if (gw == 0 && num_tiles > 0) {
       // clear the counters and the exit count, then publish: see kFusedReady
       for (int i = lane; i < p.ngroups; i += 32) p.ready[i] = 0u;
@@ -578,12 +595,16 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       float m = 0.0f;
       if (mode == 0) {
 #pragma unroll 1
-        for (int c0 = 0; c0 < nvl; c0 += kQC)
-          quant_chunk<0, 0>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
+          quant_chunk<0, 0, false, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+      } else if (mode == 3) {
+#pragma unroll 1
+        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
+          quant_chunk<0, 0, true, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
       } else if (mode == 1) {
 #pragma unroll 1
         for (int c0 = 0; c0 < nvl; c0 += kQC)
-          quant_chunk<0, 128>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+          quant_chunk<0, 128, false, kQC>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
       } else {
 #pragma unroll 1
         for (int j = 0; j < nvl; ++j)
@@ -595,12 +616,16 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       const float inv = qm::reciprocal(st);
       if (mode == 0) {
 #pragma unroll 1
-        for (int c0 = 0; c0 < nvl; c0 += kQC)
-          quant_chunk<1, 0>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
+          quant_chunk<1, 0, false, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+      } else if (mode == 3) {
+#pragma unroll 1
+        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
+          quant_chunk<1, 0, true, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
       } else if (mode == 1) {
 #pragma unroll 1
         for (int c0 = 0; c0 < nvl; c0 += kQC)
-          quant_chunk<1, 128>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+          quant_chunk<1, 128, false, kQC>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
       } else {
 #pragma unroll 1
         for (int j = 0; j < nvl; ++j)
