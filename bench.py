@@ -342,9 +342,10 @@ def run_gpu(args):
     # median 1350 MHz); this step runs for tens of ms at the full SM clock, the regime of the "burst"
     # figure.  Use burst when the sampled clock sits at the maximum, sustained otherwise, and print
     # the fraction of the other one and of the nominal peak beside it.
-    at_max = bool(clocks.get("sm_mhz") and clocks.get("sm_max_mhz") and
-                  clocks["sm_mhz"] >= 0.95 * clocks["sm_max_mhz"])
-    which = "burst" if at_max else "sustained"
+    # Fixed denominator: the timed region lasts tens of ms, the regime of the burst figure; the 4-s
+    # sustained figure (power-capped clocks) is not a ceiling for it (frac_of_2x_bf16_sustained > 1)
+    # and is printed beside it, as is the sustained leg's own rate further down.
+    which = "burst"
     int8_peak = 2.0 * peaks["bf16_" + which]
     traffic, traffic_source = stored_traffic("w4a4_gemm_kernel")
     roofline = {"bound": "tensor", "kernel": "w4a4_gemm_kernel", "achieved": tops, "peak": int8_peak,
@@ -467,6 +468,7 @@ def run_fused(args, bq, torch, plan, acts, layers, T):
     same inputs; the two-kernel time beside it is quantiser + GEMM of the timed step."""
     steps = max(3, min(args.steps, 20))
     out = []
+    time.sleep(1.0)        # the sustained leg just ran into the power cap: let the clocks come back
     for act, specs in plan:
         a = acts[act]
         for sp in specs:
