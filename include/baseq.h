@@ -169,7 +169,7 @@ BASEQ_API baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scal
  * epilogue adds the lower-bound term:  Y = bf16_rne( fma(s_t s_w, acc, fma(z_t s_w, wsum[n], fb[n])) )
  * with wsum[n] = sum_k qw[n,k] from the packed blob (fp64 expression, one rounding to bf16).
  * Scalar gamma or the per-channel vector p->sa, any K the symmetric call accepts; there is no
- * fused (quantise-in-producer) variant with asymmetric codes. */
+ * fused (single-launch) variant with asymmetric codes. */
 BASEQ_API baseq_status_t baseq_quantize_act_asym(const void* x_bf16, int64_t ldx, int T, int K,
                                        const baseq_act_params_t* p, uint8_t* codes, float* scales,
                                        float* zeros, void* stream);
