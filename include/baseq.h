@@ -206,7 +206,9 @@ BASEQ_API baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int 
  *                last CTA resets (memory that was never a workspace carries that word by chance
  *                with probability 2^-64); nothing but the kernel is enqueued, so the call can be
  *                captured in a CUDA graph and replayed.  It may be reused by the next call on the
- *                same stream; two calls that overlap on the GPU must not share it
+ *                same stream; two calls that overlap on the GPU must not share it (with
+ *                workspaces of their own they may overlap: the quantiser warps claim token rows
+ *                from a counter, so a CTA that is resident never waits for one that is not)
  *   codes_dump   optional [T, K/2]: the codes are written there instead of the workspace, or NULL
  *   scales_out   [T] required                                                                */
 BASEQ_API size_t baseq_fused_workspace_bytes(int T, int N, int K);

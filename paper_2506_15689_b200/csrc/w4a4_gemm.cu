@@ -143,7 +143,7 @@ struct GemmParams {
   float* scales_out;        // [T] (= scales)
   unsigned int* ready;      // [ceil(T / 128)] rows quantised per 128-row group
   unsigned long long* ctrl; // workspace control block: [0] = kFusedReady once the counters are zero,
-                            // [1] (low word) = CTAs that have finished
+                            // [1] (low word) = CTAs that have finished, [2] = next row to quantise
   int ngroups;
 };
 
@@ -560,9 +560,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     }
   } else if (FUSED && warp < C::kQuantWarp0 + kQuantWarps) {
     // ===================================================================== background quantiser
-    // One token row per warp (rows gw, gw + 4 * gridDim.x, ...: 256-row strips complete in the
-    // order the M-major tile walk needs them).  Lane l owns the 16-byte vectors l, l + 32, ... of
-    // the row, so an aligned half-warp holds 128 consecutive channels (what qm::hadamard8's shuffle
+    // One token row per warp, claimed from a counter (see below).  Lane l owns the 16-byte vectors
+    // l, l + 32, ... of the row, so an aligned half-warp holds 128 consecutive channels (what qm::hadamard8's shuffle
     // stages expect; a 256-channel block spans the warp).  Same arithmetic (quant_math.cuh) and
     // therefore the same codes as the stand-alone quantiser.  Two passes over the row -- absmax,
     // then round and pack; the second one re-reads the row from L2 and recomputes u.  No
@@ -570,7 +569,6 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     // limit, and it leaves 40 % of the issue slots and most of HBM idle.
     ptx::setmaxnreg_inc<128>();
     const int gw = static_cast<int>(blockIdx.x) * kQuantWarps + (warp - C::kQuantWarp0);
-    const int gws = static_cast<int>(gridDim.x) * kQuantWarps;
     const int nv = p.K >> 3;
     const int nvl = (nv + 31) >> 5;                   // vectors per lane (the last one may be idle)
     // 0 / 1: pipelined chunks without / with the block-128 Hadamard; 3: as 0 with the bf16 fma
@@ -581,15 +579,37 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     if (gw == 0 && num_tiles > 0) {
       // clear the counters and the exit count, then publish: see kFusedReady
       for (int i = lane; i < p.ngroups; i += 32) p.ready[i] = 0u;
-      if (lane == 0) p.ctrl[1] = 0ull;
+      if (lane == 0) {
+        p.ctrl[1] = 0ull;          // CTAs that have finished
+        p.ctrl[2] = 0ull;          // next token row to quantise
+      }
       __syncwarp();
       if (lane == 0) {
         __threadfence();
         ptx::st_release_gpu_u64(p.ctrl, kFusedReady);
       }
     }
-    bool seen_ready = false;
-    for (int row = gw; row < p.T && num_tiles > 0; row += gws) {
+    // Rows are CLAIMED, not assigned: a warp takes the next row from a counter in the control block
+    // (in increasing order, so 256-row strips complete in the order the tile walk needs them).  With
+    // a static assignment the GEMM warps of a resident CTA would wait for rows owned by a CTA that
+    // is not resident yet -- a second spin-waiting kernel on another stream holding the remaining SMs
+    // would then deadlock both.  Claimed rows need nothing from a CTA that is not running (CTA 0,
+    // which clears the control block, is the first to be placed).  The claim for the next row is
+    // issued before the current one is processed, so its L2 round trip is hidden; the first one costs
+    // the launch about 2 us (measured against the static assignment: c3 up 135.7 -> 138.7 us; long
+    // rows gain from the balancing: c3 down 162.6 -> 158.3 us).
+    unsigned int* next_row = reinterpret_cast<unsigned int*>(p.ctrl + 2);
+    int row = p.T;
+    if (num_tiles > 0) {
+      if (lane == 0) {
+        fused_wait_ready(p.ctrl);
+        row = static_cast<int>(atomicAdd(next_row, 1u));
+      }
+      row = __shfl_sync(0xffffffffu, row, 0);
+    }
+    while (row < p.T) {
+      int claimed = 0;
+      if (lane == 0) claimed = static_cast<int>(atomicAdd(next_row, 1u));
       const uint4* xr = p.x + static_cast<int64_t>(row) * p.ldxv;
       uint32_t* cr = p.codes_out + static_cast<int64_t>(row) * nv;
       float m = 0.0f;
@@ -633,11 +653,8 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       }
       if (lane == 0) p.scales_out[row] = st;
       __syncwarp();
-      if (lane == 0) {
-        if (!seen_ready) fused_wait_ready(p.ctrl);
-        ptx::red_release_gpu_add(p.ready + (row >> 7), 1u);
-      }
-      seen_ready = true;
+      if (lane == 0) ptx::red_release_gpu_add(p.ready + (row >> 7), 1u);
+      row = __shfl_sync(0xffffffffu, claimed, 0);
     }
   } else if (warp >= kAWarp0 && warp < kAWarp0 + 8) {
     // ===================================================================== A: smem -> TMEM
