@@ -415,6 +415,32 @@ def test_fused_workspace_is_reused_without_clearing():
     assert np.array_equal(ws[off:].cpu().numpy().reshape(T, K // 2), ref["codes"])
 
 
+def test_fused_launches_overlapping_on_two_streams():
+    # two fused launches in flight at once, each with its own workspace: neither fits the GPU next
+    # to the other, so CTAs of both wait for SMs while resident ones wait for quantised rows --
+    # rows are claimed, so nobody waits for a CTA that is not running (w4a4_gemm.cu)
+    rng = np.random.default_rng(2024)
+    cases = []
+    for T, K, N in ((1536, 1024, 4096), (1100, 2048, 4800)):
+        x_bits = rand_x(rng, T, K)
+        W = _rand_w(rng, N, K)
+        b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+        fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+        pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(b), dev(W["layer_bias"]))
+        ref = oracle.linear(x_bits, W["w_nibbles"], W["w_scale"], fb, 0.9, 1.0, None, b, 0)
+        ws = torch.empty(bq.lib().baseq_fused_workspace_bytes(T, N, K), dtype=torch.uint8, device="cuda")
+        cases.append((bf16_dev(x_bits), bq.ActParams(0.9, 1.0, None, dev(b), 0), pw, ws, ref,
+                      torch.empty((T, N), dtype=torch.bfloat16, device="cuda"), torch.cuda.Stream()))
+    torch.cuda.synchronize()
+    for _ in range(10):
+        for x, params, pw, ws, ref, y, stream in cases:
+            with torch.cuda.stream(stream):
+                bq.linear_fused(x, params, pw, y, workspace=ws)
+    torch.cuda.synchronize()
+    for x, params, pw, ws, ref, y, stream in cases:
+        assert np.array_equal(bits_host(y), ref["y"])
+
+
 # ------------------------------------------------------------------------------- full BASELINE sizes
 # Launch configuration = the one bench.py times (full T, N, K; the timed output comes from a call
 # without dumps).  Three layers of comparison, so that every tile, both CTAs of every pair and every
