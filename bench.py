@@ -524,8 +524,18 @@ def run_asym(args, bq, torch, plan, acts, layers, T):
             total += ms
             out.append({"kind": "gemm_asym", "name": sp.name, "ms": ms,
                         "TOP_per_s": 2.0 * T * sp.N * sp.K / (ms * 1e-3) / 1e12})
+            # the same layer as ONE launch (baseq_linear_fused_asym), same bits
+            ws = torch.empty(bq.lib().baseq_fused_workspace_bytes(T, sp.N, sp.K), dtype=torch.uint8,
+                             device="cuda")
+            yf, sf, zf = torch.empty_like(L["y"]), torch.empty_like(scales), torch.empty_like(zeros)
+            fms = timed(lambda: bq.linear_fused_asym(a["x"], a["params"], L["pw"], yf, scales=sf, zeros=zf,
+                                                     workspace=ws))
+            out.append({"kind": "fused_asym", "name": sp.name, "ms": fms,
+                        "same_bits_as_two_kernel_path": bool(torch.equal(yf.view(torch.int16),
+                                                                         y.view(torch.int16)))})
     return {"kernels": out, "ms_per_step": total, "tokens_per_s": T / (total * 1e-3),
-            "note": "each kernel timed alone (warm L2 for the quantiser input at small K)"}
+            "note": "each kernel timed alone (warm L2 for the quantiser input at small K); fused_asym "
+                    "entries are the single-launch variant of the same layer, not part of ms_per_step"}
 
 
 def run_kv(args, bq, torch, T, hbm_gbs):

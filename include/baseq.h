@@ -169,7 +169,7 @@ BASEQ_API baseq_status_t baseq_w4a4_gemm(const uint8_t* codes, const float* scal
  * epilogue adds the lower-bound term:  Y = bf16_rne( fma(s_t s_w, acc, fma(z_t s_w, wsum[n], fb[n])) )
  * with wsum[n] = sum_k qw[n,k] from the packed blob (fp64 expression, one rounding to bf16).
  * Scalar gamma or the per-channel vector p->sa, any K the symmetric call accepts; there is no
- * fused (single-launch) variant with asymmetric codes. */
+ * fused single-launch variant with asymmetric codes is baseq_linear_fused_asym below. */
 BASEQ_API baseq_status_t baseq_quantize_act_asym(const void* x_bf16, int64_t ldx, int T, int K,
                                        const baseq_act_params_t* p, uint8_t* codes, float* scales,
                                        float* zeros, void* stream);
@@ -217,6 +217,16 @@ BASEQ_API baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int
                                   void* y_bf16, int64_t ldy, void* workspace, size_t workspace_bytes,
                                   uint8_t* codes_dump, float* scales_out, int32_t* acc_dump,
                                   void* stream);
+
+/* The same single launch with per-token ASYMMETRIC activations (NEXT-1; Eq. 4): the
+ * background warps quantise as baseq_quantize_act_asym does, the GEMM and epilogue are those of
+ * baseq_w4a4_gemm_asym -- the same bits as the two calls.  zeros_out [T] required (the lattice
+ * lower bounds z_t); codes_dump, if given, receives the UNSIGNED nibbles. */
+BASEQ_API baseq_status_t baseq_linear_fused_asym(const void* x_bf16, int64_t ldx, int T, int K,
+                                  const baseq_act_params_t* p, const void* packed_w, int N,
+                                  void* y_bf16, int64_t ldy, void* workspace, size_t workspace_bytes,
+                                  uint8_t* codes_dump, float* scales_out, float* zeros_out,
+                                  int32_t* acc_dump, void* stream);
 
 /* ---- end-to-end helper with HOST activations / outputs (bench.py's e2e leg) ----
  * Copies x_host (pinned or pageable) to the device scratch, runs quantize_act + w4a4_gemm on

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     lib_path,
     linear,
     linear_fused,
+    linear_fused_asym,
     linear_host,
     linear_host_scratch_bytes,
     linear_static,

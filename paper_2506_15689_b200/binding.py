@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "baseq_set_fused_bias", "baseq_quantize_act", "baseq_quantize_act_tc", "baseq_w4a4_gemm",
     "baseq_fused_workspace_bytes", "baseq_linear_fused", "baseq_linear_host_scratch_bytes",
     "baseq_linear_host", "baseq_quantize_act_asym", "baseq_w4a4_gemm_asym", "baseq_quantize_kv",
-    "baseq_linear_static_scratch_bytes", "baseq_linear_static",
+    "baseq_linear_static_scratch_bytes", "baseq_linear_static", "baseq_linear_fused_asym",
 ]
 
 
@@ -69,6 +69,9 @@ def lib():
         L.baseq_linear_fused.restype = i32
         L.baseq_linear_fused.argtypes = [vp, i64, i32, i32, c.POINTER(_ActParamsC), vp, i32, vp,
                                          i64, vp, sz, vp, vp, vp, vp]
+        L.baseq_linear_fused_asym.restype = i32
+        L.baseq_linear_fused_asym.argtypes = [vp, i64, i32, i32, c.POINTER(_ActParamsC), vp, i32, vp,
+                                              i64, vp, sz, vp, vp, vp, vp, vp]
         L.baseq_linear_host_scratch_bytes.restype = sz
         L.baseq_linear_host_scratch_bytes.argtypes = [i32, i32, i32]
         L.baseq_linear_host.restype = i32
@@ -251,6 +254,28 @@ def linear_fused(x, params, pw, y=None, codes_dump=None, acc_dump=None, scales=N
                                 _p(y), y.stride(0), _p(ws), ws.numel(), _p(codes_dump), _p(scales),
                                 _p(acc_dump), _stream()), "baseq_linear_fused")
     return y, scales
+
+
+def linear_fused_asym(x, params, pw, y=None, codes_dump=None, acc_dump=None, scales=None, zeros=None,
+                      workspace=None):
+    """Fused single-launch variant with per-token asymmetric activations.  Returns (y, scales, zeros)."""
+    T, K = x.shape
+    L = lib()
+    if y is None:
+        y = torch.empty((T, pw.N), dtype=torch.bfloat16, device=x.device)
+    if scales is None:
+        scales = torch.empty((T,), dtype=torch.float32, device=x.device)
+    if zeros is None:
+        zeros = torch.empty((T,), dtype=torch.float32, device=x.device)
+    ws = workspace
+    if ws is None:
+        ws = torch.empty(max(L.baseq_fused_workspace_bytes(T, pw.N, K), 256), dtype=torch.uint8,
+                         device=x.device)
+    cs = params.c_struct()
+    _check(L.baseq_linear_fused_asym(_p(x), x.stride(0), T, K, ctypes.byref(cs), _p(pw.blob), pw.N,
+                                     _p(y), y.stride(0), _p(ws), ws.numel(), _p(codes_dump), _p(scales),
+                                     _p(zeros), _p(acc_dump), _stream()), "baseq_linear_fused_asym")
+    return y, scales, zeros
 
 
 def linear_host(x_host, params, pw, y_host, scratch):

@@ -370,6 +370,38 @@ baseq_status_t baseq_linear_fused(const void* x_bf16, int64_t ldx, int T, int K,
   return from_cuda(launch_linear_fused(g));
 }
 
+baseq_status_t baseq_linear_fused_asym(const void* x_bf16, int64_t ldx, int T, int K,
+                                       const baseq_act_params_t* p, const void* packed_w, int N,
+                                       void* y_bf16, int64_t ldy, void* workspace, size_t workspace_bytes,
+                                       uint8_t* codes_dump, float* scales_out, float* zeros_out,
+                                       int32_t* acc_dump, void* stream) {
+  if (workspace == nullptr || zeros_out == nullptr) return BASEQ_ERR_NULL;
+  baseq_status_t st = validate_quant(x_bf16, ldx, T, K, p, codes_dump, scales_out, false);
+  if (st != BASEQ_OK) return st;
+  st = validate_gemm(nullptr, scales_out, packed_w, T, N, K, y_bf16, ldy, acc_dump, false);
+  if (st != BASEQ_OK) return st;
+  if (!aligned(workspace, 256) || !aligned(zeros_out, 4)) return BASEQ_ERR_ALIGN;
+  if (workspace_bytes < baseq_fused_workspace_bytes(T, N, K)) return BASEQ_ERR_WORKSPACE;
+  if (!fused_supported(p->had_block)) return BASEQ_ERR_UNSUPPORTED;
+  DeviceRef d;
+  st = device_check(&d);
+  if (st != BASEQ_OK) return st;
+  GemmLaunch g = make_gemm(nullptr, scales_out, zeros_out, packed_w, T, N, K, y_bf16, ldy, acc_dump, stream, d);
+  g.x = x_bf16;
+  g.ldx = ldx;
+  g.alpha = p->alpha;
+  g.gamma = p->gamma;
+  g.sa = p->sa;
+  g.b = p->b;
+  g.had_block = p->had_block;
+  g.had_scale = p->had_block
+                    ? static_cast<float>(1.0 / std::sqrt(static_cast<double>(p->had_block)))
+                    : 1.0f;
+  g.codes_dump = codes_dump;
+  g.workspace = workspace;
+  return from_cuda(launch_linear_fused(g));
+}
+
 size_t baseq_linear_host_scratch_bytes(int T, int N, int K) {
   if (check_shape(T, N, K) != BASEQ_OK) return 0;
   auto up = [](size_t v) { return (v + 255) / 256 * 256; };

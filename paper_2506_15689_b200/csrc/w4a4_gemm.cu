@@ -141,6 +141,7 @@ struct GemmParams {
   float had_scale;
   uint32_t* codes_out;      // [T, K/8] words of 8 nibbles: the workspace (or the caller's codes_dump)
   float* scales_out;        // [T] (= scales)
+  float* zeros_out;         // [T] (= zeros; asymmetric fused variant)
   unsigned int* ready;      // [ceil(T / 128)] rows quantised per 128-row group
   unsigned long long* ctrl; // workspace control block: [0] = kFusedReady once the counters are zero,
                             // [1] (low word) = CTAs that have finished, [2] = next row to quantise
@@ -238,15 +239,18 @@ __device__ __forceinline__ void dequant_bracket_asym(int32_t raw, float st256, f
 constexpr int kQD = 4;     // ring slots = loads in flight per lane: x + 2 x b per slot
 constexpr int kQC = 8;     // vector steps per chunk (16 without the Hadamard measured 4 % slower for
                            // the whole launch on K = 4096: twice the code in the instruction cache)
-constexpr int kQCLong = kQC;
 // GBF16 (HAD == 0 only): the scalar s^a is a bf16 value, so Q0 + Q2 are ONE mixed-precision fma per
 // element (as in the stand-alone quantiser, quant_math.cuh) -- computed as -u = fma(x, -gamma, b),
 // which needs no negated copy of b; |-u| = |u| for the absmax, and pass 1 rounds (-u) * (-inv), the
 // same exact product as u * inv.
-template <int PASS, int HAD, bool GBF16, int QC>
+// AQ (NEXT-1): per-token asymmetric codes -- pass 0 tracks max u (m) and max -u (m2), pass 1 rounds
+// (u - z) * inv to 0 .. 15 (quant_math.cuh A1-A3).  With GBF16 the chunk holds -u: the two maxima
+// swap roles, and (-u) - (-z) = -(u - z) times -inv is the same exact product.
+template <int PASS, int HAD, bool GBF16, int QC, bool AQ>
 __device__ __forceinline__ void quant_chunk(const uint4* __restrict__ xr, const float* __restrict__ bvec,
                                             float gamma, float had_scale, int lane, int nv, int nvl,
-                                            int c0, float inv, float& m, uint32_t* __restrict__ cr) {
+                                            int c0, float inv, float z, float& m, float& m2,
+                                            uint32_t* __restrict__ cr) {
   static_assert(!(GBF16 && HAD != 0), "the bf16 fma consumes the packed activations as they are");
   uint4 sx[kQD];
   float4 sb0[kQD], sb1[kQD];
@@ -285,21 +289,30 @@ __device__ __forceinline__ void quant_chunk(const uint4* __restrict__ xr, const 
       for (int e = 0; e < 8; ++e) u[e] = qm::affine(gamma, f[e], bb[e]);
     }
     if (PASS == 0) {
-      const float mm = qm::absmax8(m, u);
-      m = valid ? mm : m;
+      if (AQ) {
+        float mx = m, mn = m2;
+        if (GBF16) qm::maxmin8(mn, mx, u);
+        else qm::maxmin8(mx, mn, u);
+        m = valid ? mx : m;
+        m2 = valid ? mn : m2;
+      } else {
+        const float mm = qm::absmax8(m, u);
+        m = valid ? mm : m;
+      }
     } else {
-      const uint32_t w = qm::quantize_pack8(u, GBF16 ? -inv : inv);
+      const uint32_t w = AQ ? qm::quantize_pack8_asym(u, GBF16 ? -z : z, GBF16 ? -inv : inv)
+                            : qm::quantize_pack8(u, GBF16 ? -inv : inv);
       if (valid) cr[i] = w;
     }
     if (t + kQD < QC) issue(d, j + kQD);
   }
 }
 // Any parameter combination, one vector step at a time (loads not pipelined).
-template <int PASS>
+template <int PASS, bool AQ>
 __device__ __forceinline__ void quant_step_generic(const uint4* __restrict__ xr, const float* __restrict__ bvec,
                                                    const float* __restrict__ sa, float gamma, int had_block,
                                                    float had_scale, int lane, int nv, int j, float inv,
-                                                   float& m, uint32_t* __restrict__ cr) {
+                                                   float z, float& m, float& m2, uint32_t* __restrict__ cr) {
   const int i = lane + 32 * j;
   const bool ok = i < nv;
   const uint4 v = ok ? __ldg(xr + i) : make_uint4(0u, 0u, 0u, 0u);
@@ -310,8 +323,12 @@ __device__ __forceinline__ void quant_step_generic(const uint4* __restrict__ xr,
 #pragma unroll
   for (int e = 0; e < 8; ++e) u[e] = qm::affine(g[e], f[e], bb[e]);
   if (ok) {
-    if (PASS == 0) m = qm::absmax8(m, u);
-    else cr[i] = qm::quantize_pack8(u, inv);
+    if (PASS == 0) {
+      if (AQ) qm::maxmin8(m, m2, u);
+      else m = qm::absmax8(m, u);
+    } else {
+      cr[i] = AQ ? qm::quantize_pack8_asym(u, z, inv) : qm::quantize_pack8(u, inv);
+    }
   }
 }
 
@@ -612,45 +629,51 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
       if (lane == 0) claimed = static_cast<int>(atomicAdd(next_row, 1u));
       const uint4* xr = p.x + static_cast<int64_t>(row) * p.ldxv;
       uint32_t* cr = p.codes_out + static_cast<int64_t>(row) * nv;
-      float m = 0.0f;
+      // symmetric: m = max |u|; asymmetric: m = max u, m2 = max -u
+      float m = ASYM ? -3.402823466e38f : 0.0f, m2 = -3.402823466e38f;
       if (mode == 0) {
 #pragma unroll 1
-        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
-          quant_chunk<0, 0, false, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<0, 0, false, kQC, ASYM>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, 0.0f, m, m2, cr);
       } else if (mode == 3) {
 #pragma unroll 1
-        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
-          quant_chunk<0, 0, true, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<0, 0, true, kQC, ASYM>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, 0.0f, m, m2, cr);
       } else if (mode == 1) {
 #pragma unroll 1
         for (int c0 = 0; c0 < nvl; c0 += kQC)
-          quant_chunk<0, 128, false, kQC>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, m, cr);
+          quant_chunk<0, 128, false, kQC, ASYM>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, 0.0f, 0.0f, m, m2, cr);
       } else {
 #pragma unroll 1
         for (int j = 0; j < nvl; ++j)
-          quant_step_generic<0>(xr, p.bvec, p.sa, p.gamma, p.had_block, p.had_scale, lane, nv, j, 0.0f, m, cr);
+          quant_step_generic<0, ASYM>(xr, p.bvec, p.sa, p.gamma, p.had_block, p.had_scale, lane, nv, j, 0.0f, 0.0f, m, m2, cr);
       }
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-      const float st = qm::step_size(p.alpha, m);
+      for (int o = 16; o > 0; o >>= 1) {
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (ASYM) m2 = fmaxf(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+      }
+      const float st = ASYM ? qm::step_size_asym(p.alpha, -m2, m) : qm::step_size(p.alpha, m);
+      const float zt = ASYM ? qm::lower_bound_asym(p.alpha, -m2) : 0.0f;
       const float inv = qm::reciprocal(st);
       if (mode == 0) {
 #pragma unroll 1
-        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
-          quant_chunk<1, 0, false, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<1, 0, false, kQC, ASYM>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, zt, m, m2, cr);
       } else if (mode == 3) {
 #pragma unroll 1
-        for (int c0 = 0; c0 < nvl; c0 += kQCLong)
-          quant_chunk<1, 0, true, kQCLong>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+        for (int c0 = 0; c0 < nvl; c0 += kQC)
+          quant_chunk<1, 0, true, kQC, ASYM>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, zt, m, m2, cr);
       } else if (mode == 1) {
 #pragma unroll 1
         for (int c0 = 0; c0 < nvl; c0 += kQC)
-          quant_chunk<1, 128, false, kQC>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, m, cr);
+          quant_chunk<1, 128, false, kQC, ASYM>(xr, p.bvec, p.gamma, p.had_scale, lane, nv, nvl, c0, inv, zt, m, m2, cr);
       } else {
 #pragma unroll 1
         for (int j = 0; j < nvl; ++j)
-          quant_step_generic<1>(xr, p.bvec, p.sa, p.gamma, p.had_block, p.had_scale, lane, nv, j, inv, m, cr);
+          quant_step_generic<1, ASYM>(xr, p.bvec, p.sa, p.gamma, p.had_block, p.had_scale, lane, nv, j, inv, zt, m, m2, cr);
       }
+      if (ASYM && lane == 0) p.zeros_out[row] = zt;
       if (lane == 0) p.scales_out[row] = st;
       __syncwarp();
       if (lane == 0) ptx::red_release_gpu_add(p.ready + (row >> 7), 1u);
@@ -763,7 +786,7 @@ w4a4_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         st = p.scales[row];
       }
       const float st256 = __fmul_rn(st, 0.00390625f);
-      const float zt = (ASYM && row_ok) ? p.zeros[row] : 0.0f;
+      const float zt = (ASYM && row_ok) ? (FUSED ? ptx::ld_relaxed_gpu_f32(p.zeros + row) : p.zeros[row]) : 0.0f;
       const float midf = __fmaf_rn(8.0f, st, zt);
       float* cs = colp + as * 3 * BN;
 #pragma unroll
@@ -1021,7 +1044,7 @@ cudaError_t launch_pair(const CUtensorMap& tmap_a, const CUtensorMap& tmap_y, co
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
   const bool fused = g.x != nullptr;
   if (!fused && g.T <= kDecodeMaxT) return launch_w4a4_decode(g);   // decode shapes: W-streaming kernel
-  if (fused && (!fused_supported(g.had_block) || g.zeros != nullptr)) return cudaErrorNotSupported;
+  if (fused && !fused_supported(g.had_block)) return cudaErrorNotSupported;
   const BlobHeader h = blob_header(g.N, g.K);
   const uint8_t* base = static_cast<const uint8_t*>(g.blob);
 
@@ -1074,9 +1097,11 @@ cudaError_t launch_w4a4_gemm(const GemmLaunch& g) {
     p.had_scale = g.had_scale;
     p.codes_out = reinterpret_cast<uint32_t*>(const_cast<uint8_t*>(codes));
     p.scales_out = const_cast<float*>(g.scales);
+    p.zeros_out = const_cast<float*>(g.zeros);
     p.ctrl = reinterpret_cast<unsigned long long*>(wsb);
     p.ready = reinterpret_cast<unsigned int*>(wsb + ws.off_ready);
     p.ngroups = ws.ngroups;
+    if (g.zeros != nullptr) return launch_pair<true, true>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
     return launch_pair<true, false>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);
   }
   if (g.zeros != nullptr) return launch_pair<false, true>(tmap_a, tmap_y, p, g.num_sms, g.device, g.stream);

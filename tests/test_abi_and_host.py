@@ -94,6 +94,13 @@ def test_validation_happens_before_any_launch():
              None) == 4
     assert f(base, 256, 4, 256, ctypes.byref(ok), base, 12, base, 16, base, 4096, None, base, None,
              None) == 2                                                            # N % 8 (second stage)
+    fa = L.baseq_linear_fused_asym
+    assert fa(base, 256, 4, 256, ctypes.byref(ok), base, 8, base, 8, base, 4096, None, base, None, None,
+              None) == 1                                                           # zeros_out required
+    assert fa(base, 256, 4, 256, ctypes.byref(bad_alpha), base, 8, base, 8, base, 4096, None, base, base,
+              None, None) == 4
+    assert fa(base, 256, 4, 256, ctypes.byref(ok), base, 8, base, 8, base, 512, None, base, base, None,
+              None) == 5
     h = L.baseq_linear_host
     assert h(base, 4, 256, ctypes.byref(bad_alpha), base, 8, base, base, 1 << 20, None) == 4
     assert h(base, 4, 65536, ctypes.byref(ok), base, 8, base, base, 1 << 30, None) == 2

@@ -775,6 +775,69 @@ def run_asym(x_bits, W, alpha, gamma, b, had_block=0, rows=None, sa=None):
     assert nbad == 0, "asym bf16 output differs at %d of %d places" % (nbad, gy.size)
 
 
+def run_fused_asym(x_bits, W, alpha, gamma, b, had_block=0, sa=None):
+    """baseq_linear_fused_asym vs the oracle AND vs the two asymmetric calls, everything bit for bit."""
+    N, K = W["N"], W["K"]
+    T = x_bits.shape[0]
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), None if b is None else dev(b),
+                         None if W["layer_bias"] is None else dev(W["layer_bias"]))
+    params = bq.ActParams(alpha, gamma, None if sa is None else dev(sa), None if b is None else dev(b),
+                          had_block)
+    x = bf16_dev(x_bits)
+    codes = torch.zeros((T, K // 2), dtype=torch.uint8, device="cuda")
+    acc = torch.empty((T, N), dtype=torch.int32, device="cuda")
+    y, scales, zeros = bq.linear_fused_asym(x, params, pw, codes_dump=codes, acc_dump=acc)
+    y2, _, _ = bq.linear_fused_asym(x, params, pw)                    # timed configuration: no dumps
+    c3, s3, z3 = bq.quantize_act_asym(x, params)
+    y3 = bq.w4a4_gemm_asym(c3, s3, z3, pw)
+    torch.cuda.synchronize()
+    assert torch.equal(y.view(torch.int16), y2.view(torch.int16))
+    assert torch.equal(y.view(torch.int16), y3.view(torch.int16))
+    assert torch.equal(codes, c3) and torch.equal(scales, s3) and torch.equal(zeros, z3)
+    ref = oracle.linear_asym(x_bits, W["w_nibbles"], W["w_scale"], fb, alpha, gamma, sa, b, had_block)
+    assert np.array_equal(scales.cpu().numpy().view(np.uint32), ref["scales"].view(np.uint32))
+    assert np.array_equal(zeros.cpu().numpy().view(np.uint32), ref["zeros"].view(np.uint32))
+    assert np.array_equal(codes.cpu().numpy(), ref["codes"])
+    assert np.array_equal(acc.cpu().numpy(), ref["acc"])
+    assert np.array_equal(bits_host(y), ref["y"])
+
+
+@pytest.mark.parametrize("T,K,N,B", [(1, 128, 8, 0), (130, 384, 264, 0), (257, 1024, 520, 128),
+                                     (300, 2048, 200, 16), (700, 4096, 392, 0), (520, 1280, 136, 256)])
+def test_fused_asym_shapes(T, K, N, B):
+    # the single-launch variant with asymmetric activations: pipelined chunks with and without the
+    # Hadamard-128, generic steps (other block sizes), gamma a bf16 value and not
+    rng = np.random.default_rng(31 * T + 3 * K + 5 * N + B)
+    x = rand_x(rng, T, K, spread=1.0)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    run_fused_asym(x, _rand_w(rng, N, K), 0.9, 1.0 if T % 2 else 1.05, b, had_block=B)
+
+
+def test_fused_asym_per_channel_sa_and_offsets():
+    rng = np.random.default_rng(41)
+    T, K, N = 70, 512, 136
+    x = f32_to_bf16_bits((5.0 + rng.standard_normal((T, K))).astype(np.float32))     # far from zero
+    sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+    run_fused_asym(x, _rand_w(rng, N, K, bias=False), 1.0, 1.0, None, sa=sa)
+
+
+def test_fused_asym_full_size_c3_up():
+    L = cached_layer("c3", "up")
+    sp = L["spec"]
+    pw = bq.pack_weights(dev(L["w_nibbles"]), dev(L["w_scale"]), dev(L["b"]),
+                         None if L["layer_bias"] is None else dev(L["layer_bias"]))
+    params = bq.ActParams(sp.alpha, sp.gamma, None, dev(L["b"]), sp.had_block)
+    x = bf16_dev(L["x"])
+    y, scales, zeros = bq.linear_fused_asym(x, params, pw)
+    c3, s3, z3 = bq.quantize_act_asym(x, params)
+    y3 = bq.w4a4_gemm_asym(c3, s3, z3, pw)
+    torch.cuda.synchronize()
+    # the two-call path is checked against the oracle at full size by test_full_size_asym
+    assert torch.equal(scales, s3) and torch.equal(zeros, z3)
+    assert torch.equal(y.view(torch.int16), y3.view(torch.int16))
+
+
 def test_asym_config1():
     L = make_layer("c1", "linear")
     sp = L["spec"]
