@@ -14,7 +14,6 @@
 // place), three-input max (FMNMX3), fma-with-magic rounding and the saturating nibble pack the two
 // passes cost 4 issue slots per element (FHFMA, 1/2 FMNMX3, FFMA, IADD, 1/2 I2IP) instead of the ~9
 // of r1 (unpack, FFMA, FMNMX, FFMA, IADD, I2IP plus address arithmetic).
-#include <cstdlib>
 #include <cstring>
 
 #include "kernels.cuh"
@@ -488,8 +487,7 @@ cudaError_t launch_ring_split_g(const QuantLaunch& q, bool write_codes) {
   RingParams p = make_params(q, write_codes);
   p.stage_bytes = G * q.K * 2;
   const int sa_bytes = GMODE == kGVec ? q.K * 4 : 0;
-  const int budget = G == 4 ? kRingSmemBudget : 108 * 1024;
-  int stages = (budget - sa_bytes) / p.stage_bytes;
+  int stages = (kRingSmemBudget - sa_bytes) / p.stage_bytes;
   p.stages = stages > kMaxStages ? kMaxStages : stages;
   if (p.stages < 2) return cudaErrorInvalidValue;
   const int smem = p.stages * p.stage_bytes + sa_bytes;
@@ -503,9 +501,7 @@ cudaError_t launch_ring_split_g(const QuantLaunch& q, bool write_codes) {
 
 template <int V, bool ASYM, int GMODE>
 cudaError_t launch_ring_split(const QuantLaunch& q, bool write_codes) {
-  static const int g_exp = getenv("BASEQ_SPLIT_G") ? atoi(getenv("BASEQ_SPLIT_G")) : 4;
-  return g_exp == 2 ? launch_ring_split_g<V, 2, ASYM, GMODE>(q, write_codes)
-                    : launch_ring_split_g<V, 4, ASYM, GMODE>(q, write_codes);
+  return launch_ring_split_g<V, 4, ASYM, GMODE>(q, write_codes);
 }
 
 template <int V, int RL, bool HAD, bool RAGGED, bool ASYM, int GMODE>
