@@ -78,7 +78,9 @@ BASEQ_API baseq_status_t baseq_sync_status(void* stream);
  *   q_k = clamp(rne(u_k * (1 / s_t)), -8, 7)     product exact, one rounding     (C-5, C-6, C-17)
  * every line one correctly rounded fp32 operation. */
 typedef struct {
-  float alpha;      /* clip ratio, 2^-16 <= alpha <= 1, else BASEQ_ERR_PARAM     */
+  float alpha;      /* clip ratio, 0 < alpha <= 1, else BASEQ_ERR_PARAM; below
+                       2^-16 a plain (slow) kernel takes over that clamps before it rounds -- the
+                       same codes -- and baseq_quantize_act_tc returns BASEQ_ERR_UNSUPPORTED          */
   float gamma;      /* scalar s^a, used iff sa == NULL; must be finite and > 0                      */
   const float* sa;  /* [K] per-channel s^a, already divided by the paired scale s; or NULL          */
   const float* b;   /* [K] correction bias b^c in the scaled (and rotated) domain; NULL = 0         */

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbaseq.so")
-SOURCES = ["baseq_api.cu", "quantize_act.cu", "quantize_ring.cu", "quantize_had_tc.cu", "quantize_kv.cu", "pack_weights.cu", "w4a4_gemm.cu", "w4a4_decode.cu"]
+SOURCES = ["baseq_api.cu", "quantize_act.cu", "quantize_ring.cu", "quantize_had_tc.cu", "quantize_kv.cu", "quantize_small_alpha.cu", "pack_weights.cu", "w4a4_gemm.cu", "w4a4_decode.cu"]
 HEADERS = ["kernels.cuh", "ptx.cuh", "quant_math.cuh", "epilogue_math.cuh", os.path.join("..", "..", "include", "baseq.h")]
 
 # No --use_fast_math, no -ftz: the quantiser's fp32 contract needs IEEE ops and denormals.

@@ -73,7 +73,7 @@ baseq_status_t check_shape(int T, int N, int K) {
 
 baseq_status_t check_act_params(const baseq_act_params_t* p, int K) {
   if (p == nullptr) return BASEQ_ERR_NULL;
-  if (!(p->alpha >= 1.0f / 65536.0f) || !(p->alpha <= 1.0f)) return BASEQ_ERR_PARAM;
+  if (!(p->alpha > 0.0f) || !(p->alpha <= 1.0f)) return BASEQ_ERR_PARAM;
   if (p->sa == nullptr && (!(p->gamma > 0.0f) || !std::isfinite(p->gamma))) return BASEQ_ERR_PARAM;
   if (p->had_block != 0) {
     const int B = p->had_block;
@@ -250,7 +250,7 @@ baseq_status_t baseq_quantize_act_tc(const void* x_bf16, int64_t ldx, int T, int
                                      void* stream) {
   baseq_status_t st = validate_quant(x_bf16, ldx, T, K, p, codes, scales, true);
   if (st != BASEQ_OK) return st;
-  if (!quantize_tc_supported(K, p->had_block)) return BASEQ_ERR_UNSUPPORTED;
+  if (!quantize_tc_supported(K, p->had_block) || p->alpha < kMinFastAlpha) return BASEQ_ERR_UNSUPPORTED;
   DeviceRef d;
   st = device_check(&d);
   if (st != BASEQ_OK) return st;
@@ -310,7 +310,7 @@ baseq_status_t baseq_quantize_kv(const void* x_bf16, int64_t ldx, int T, int n_h
     return BASEQ_ERR_NULL;
   if (T < 1 || n_heads < 1 || n_heads > 65536 || T > (1 << 24)) return BASEQ_ERR_SHAPE;
   if (head_dim != 64 && head_dim != 128) return BASEQ_ERR_UNSUPPORTED;
-  if (!(alpha >= 1.0f / 65536.0f && alpha <= 1.0f)) return BASEQ_ERR_PARAM;
+  if (!(alpha > 0.0f && alpha <= 1.0f)) return BASEQ_ERR_PARAM;
   if (!aligned(x_bf16, 16) || !aligned(codes, 16) || !aligned(scales, 4) || !aligned(zeros, 4))
     return BASEQ_ERR_ALIGN;
   if (ldx < static_cast<int64_t>(n_heads) * head_dim || (ldx % 8) != 0) return BASEQ_ERR_ALIGN;

@@ -87,6 +87,10 @@ struct QuantLaunch {
   int blocks_per_sm;
 };
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes);
+// alpha < kMinFastAlpha: the fast kernels' single-fma rounding needs |u / s_t| < 2^22; a plain kernel
+// that clamps first takes over (quantize_small_alpha.cu)
+constexpr float kMinFastAlpha = 1.0f / 65536.0f;
+cudaError_t launch_quantize_small_alpha(const QuantLaunch& q, bool write_codes);
 // long rows (K >= 4096): bulk-TMA ring variant of the same contract (quantize_ring.cu)
 bool quantize_ring_supported(int K);
 cudaError_t launch_quantize_ring(const QuantLaunch& q, bool write_codes);
@@ -108,6 +112,7 @@ struct KvLaunch {
   cudaStream_t stream;
 };
 cudaError_t launch_quantize_kv(const KvLaunch& q);   // cudaErrorNotSupported: head_dim not 64 / 128
+cudaError_t launch_quantize_kv_small_alpha(const KvLaunch& q);
 
 cudaError_t launch_pack_weights(const uint8_t* w_nibbles, const float* w_scale, const float* b,
                                 const float* layer_bias, int N, int K, void* blob,

@@ -173,7 +173,8 @@ __device__ __forceinline__ uint32_t pack_nibbles(const uint32_t (&t)[8]) {
 
 
 // Q6 + Q7 for 8 channels at once.  |u * inv| <= 7 / alpha (1 + 2^-22) <= 7 * 2^16 < 2^22 because
-// |u| <= the row's absmax and the API requires alpha >= 2^-16, so fma(u, inv, 1.5 * 2^23) stays in
+// |u| <= the row's absmax and the callers run for alpha >= 2^-16 only (smaller clip ratios take
+// quantize_small_alpha.cu, which clamps u first), so fma(u, inv, 1.5 * 2^23) stays in
 // [2^23, 2^24) and rounds the exact product to the nearest integer, ties to even; the integer
 // subtract recovers the signed integer, and cvt.pack.sat.s4.s32 clamps it to [-8, 7] and packs two
 // codes per instruction:  d = (c << 8) | (sat(a) << 4) | (sat(b) & 15).

@@ -185,6 +185,7 @@ cudaError_t launch_hw(const QuantLaunch& q, int V) {
 static_assert(512 * kMaxV * 8 >= kMaxK, "a row of kMaxK channels fits 512 threads x kMaxV vectors");
 
 cudaError_t launch_quantize_act(QuantLaunch q, bool write_codes) {
+  if (q.alpha < kMinFastAlpha) return launch_quantize_small_alpha(q, write_codes);
   // the asymmetric variant (NEXT-1) lives in the ring kernels only (any K)
   if (q.asym) return launch_quantize_ring(q, write_codes);
   // long rows (every benchmark shape): bulk-TMA ring kernels; short rows: the register-resident

@@ -223,6 +223,8 @@ cudaError_t launch_lpg(const KvLaunch& q) {
 }  // namespace
 
 cudaError_t launch_quantize_kv(const KvLaunch& q) {
+  if (q.head_dim != 64 && q.head_dim != 128) return cudaErrorNotSupported;
+  if (q.alpha < kMinFastAlpha) return launch_quantize_kv_small_alpha(q);
   switch (q.head_dim) {
     case 64: return launch_lpg<8>(q);
     case 128: return launch_lpg<16>(q);

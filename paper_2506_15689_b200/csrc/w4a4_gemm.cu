@@ -1116,6 +1116,36 @@ size_t fused_workspace_bytes(int T, int N, int K) {
 
 bool fused_supported(int had_block) { return had_block <= 256; }   // a block spans at most one warp
 
-cudaError_t launch_linear_fused(const GemmLaunch& g) { return launch_w4a4_gemm(g); }
+cudaError_t launch_linear_fused(const GemmLaunch& g) {
+  if (g.alpha >= kMinFastAlpha) return launch_w4a4_gemm(g);
+  // clip ratios below 2^-16: the background quantiser rounds like the fast kernels do; quantise with
+  // the clamping kernel into the codes buffer of the call, then run the plain GEMM on it
+  const FusedWorkspace ws = fused_workspace_layout(g.T, g.K);
+  uint8_t* codes = g.codes_dump != nullptr ? g.codes_dump : static_cast<uint8_t*>(g.workspace) + ws.off_codes;
+  QuantLaunch q{};
+  q.x = g.x;
+  q.ldx = g.ldx;
+  q.T = g.T;
+  q.K = g.K;
+  q.alpha = g.alpha;
+  q.gamma = g.gamma;
+  q.sa = g.sa;
+  q.b = g.b;
+  q.had_block = g.had_block;
+  q.had_scale = g.had_scale;
+  q.codes = codes;
+  q.scales = const_cast<float*>(g.scales);
+  q.zeros = const_cast<float*>(g.zeros);
+  q.asym = g.zeros != nullptr;
+  q.stream = g.stream;
+  q.num_sms = g.num_sms;
+  q.device = g.device;
+  const cudaError_t e = launch_quantize_small_alpha(q, true);
+  if (e != cudaSuccess) return e;
+  GemmLaunch u = g;
+  u.x = nullptr;
+  u.codes = codes;
+  return launch_w4a4_gemm(u);
+}
 
 }  // namespace baseq

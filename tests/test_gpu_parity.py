@@ -938,6 +938,62 @@ def test_kv_rejects_other_head_dims():
         bq.quantize_kv(x, 2, 96)
 
 
+# ------------------------------------------------------------------------------- clip ratios below 2^-16
+def _tiny_alpha_x(rng, T, K):
+    # N(0.3, 1) rows with a fifth of the entries scaled down to the size of the step alpha * max / 7,
+    # so that codes other than the saturated ones occur
+    x = 0.3 + rng.standard_normal((T, K))
+    small = rng.random((T, K)) < 0.2
+    x[small] *= 1e-6
+    return f32_to_bf16_bits(x.astype(np.float32))
+
+
+@pytest.mark.parametrize("alpha", [2.0 ** -17, 2.0 ** -20, 1e-9])
+def test_small_alpha_every_entry_point(alpha):
+    # include/baseq.h allows 0 < alpha <= 1; below 2^-16 the clamping kernel (quantize_small_alpha.cu)
+    # takes over behind every entry point: same contract, same bits as the oracle
+    rng = np.random.default_rng(int(-np.log2(alpha)))
+    T, K, N = 75, 1024, 200
+    x = _tiny_alpha_x(rng, T, K)
+    b = (1e-7 * rng.standard_normal(K)).astype(np.float32)
+    W = _rand_w(rng, N, K)
+    for B in (0, 128, 256):
+        check_quant(x, alpha, 1.05, None, b, B)
+        run_linear(x, W, alpha, 1.0, b, had_block=B)
+        run_asym(x, W, alpha, 1.0, b, had_block=B)
+        run_fused(x, W, alpha, 1.0, b, had_block=B)
+        run_fused_asym(x, W, alpha, 1.05, b, had_block=B)
+    sa = (1.0 + 0.1 * rng.standard_normal(K)).astype(np.float32)
+    check_quant(x, alpha, 1.0, sa, None)
+    # the ring kernels' shapes route there too
+    x2 = _tiny_alpha_x(rng, 9, 11008)
+    check_quant(x2, alpha, 1.0, None, (1e-7 * rng.standard_normal(11008)).astype(np.float32))
+    # KV cache: (token, head) groups, strided rows
+    xk = _tiny_alpha_x(rng, 33, 5 * 128)
+    run_kv(xk, 5, 128, alpha)
+    run_kv(_tiny_alpha_x(rng, 17, 3 * 64), 3, 64, alpha, ldx=3 * 64 + 24)
+    # the tensor-core Hadamard variant keeps the limit
+    with pytest.raises(bq.BaseqError) as e:
+        bq.quantize_act_tc(bf16_dev(x), bq.ActParams(alpha, 1.0, None, dev(b), 128))
+    assert e.value.status == 6
+
+
+def test_small_alpha_static_entry_point():
+    rng = np.random.default_rng(5)
+    T, K, N = 40, 512, 72
+    x_bits = _tiny_alpha_x(rng, T, K)
+    W = _rand_w(rng, N, K)
+    b = (1e-7 * rng.standard_normal(K)).astype(np.float32)
+    alpha = 2.0 ** -18
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(b), dev(W["layer_bias"]))
+    y = torch.empty((T, N), dtype=torch.bfloat16, device="cuda")
+    bq.linear_static(bf16_dev(x_bits), bq.ActParams(alpha, 1.0, None, dev(b), 0), pw, y)
+    torch.cuda.synchronize()
+    ref = oracle.linear(x_bits, W["w_nibbles"], W["w_scale"], fb, alpha, 1.0, None, b, 0)
+    assert np.array_equal(bits_host(y), ref["y"])
+
+
 # ------------------------------------------------------------------------------- NEXT-4: decode shapes
 # T <= 64 takes the W-streaming decode kernel (w4a4_decode.cu) behind the same baseq_w4a4_gemm /
 # baseq_w4a4_gemm_asym calls; same contract, same bits.
