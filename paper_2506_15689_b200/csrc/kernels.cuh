@@ -129,7 +129,7 @@ struct GemmLaunch {
   void* y;                 // bf16 [T, ldy]
   int64_t ldy;
   int32_t* acc_dump;       // optional [T, N]
-  // fused producer inputs (x != nullptr selects the quantise-in-producer variant)
+  // fused single-launch variant (x != nullptr selects it): the background quantiser's inputs
   const void* x;
   int64_t ldx;
   float alpha, gamma;
@@ -146,7 +146,8 @@ struct GemmLaunch {
 };
 // Returns cudaSuccess, or an error (cudaErrorNotSupported when the tensor map cannot be built).
 cudaError_t launch_w4a4_gemm(const GemmLaunch& g);
-// Fused variant (a10): scales pre-pass + quantise-in-producer GEMM; g.x != nullptr, g.scales = scales_out.
+// Fused variant (a10): GEMM with background quantiser warps, one launch; g.x != nullptr,
+// g.scales = scales_out (g.zeros = zeros_out selects asymmetric codes).
 size_t fused_workspace_bytes(int T, int N, int K);
 bool fused_supported(int had_block);
 cudaError_t launch_linear_fused(const GemmLaunch& g);

@@ -1,5 +1,5 @@
 // The quantiser's arithmetic contract (Q0-Q7), written once and used by
-// both the stand-alone row kernel (quantize_act.cu) and the quantise-in-producer warps of the
+// both the stand-alone row kernels (quantize_act.cu, quantize_ring.cu) and the background quantiser warps of the
 // fused GEMM (w4a4_gemm.cu).  Every line is one correctly rounded fp32 operation -- explicit
 // __f*_rn intrinsics are never contracted or re-associated by nvcc.
 //

@@ -48,7 +48,7 @@ struct RingParams {
   const float* sa;         // per-channel s^a (kGVec), else NULL
   int had_block;
   float had_scale;
-  uint32_t* codes;         // NULL: scales only (the fused GEMM's absmax pre-pass)
+  uint32_t* codes;         // NULL: scales only
   float* scales;
   float* zeros;            // asymmetric variant only
   int stages;
