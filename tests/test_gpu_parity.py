@@ -415,6 +415,42 @@ def test_fused_workspace_is_reused_without_clearing():
     assert np.array_equal(ws[off:].cpu().numpy().reshape(T, K // 2), ref["codes"])
 
 
+def test_fused_and_static_calls_replay_in_a_cuda_graph():
+    # neither call enqueues anything but kernels (the fused workspace is cleared by the kernel itself,
+    # the static entry point owns its scratch): capture once, replay with new inputs in place
+    rng = np.random.default_rng(909)
+    T, K, N = 520, 1024, 392
+    W = _rand_w(rng, N, K)
+    b = (0.5 * rng.standard_normal(K)).astype(np.float32)
+    fb = oracle.fused_bias(W["w_nibbles"], W["w_scale"], b, W["layer_bias"])
+    pw = bq.pack_weights(dev(W["w_nibbles"]), dev(W["w_scale"]), dev(b), dev(W["layer_bias"]))
+    params = bq.ActParams(0.9, 1.0, None, dev(b), 0)
+    x = torch.empty((T, K), dtype=torch.bfloat16, device="cuda")
+    yf = torch.empty((T, N), dtype=torch.bfloat16, device="cuda")
+    ys = torch.empty_like(yf)
+    scales = torch.empty((T,), dtype=torch.float32, device="cuda")
+    ws = torch.full((bq.lib().baseq_fused_workspace_bytes(T, N, K),), 0xAB, dtype=torch.uint8, device="cuda")
+    xs = [rand_x(rng, T, K) for _ in range(3)]
+    stream = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(stream):
+        x.copy_(bf16_dev(xs[0]))
+        bq.linear_fused(x, params, pw, yf, scales=scales, workspace=ws)        # warm-up outside capture
+        bq.linear_static(x, params, pw, ys)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=stream):
+            bq.linear_fused(x, params, pw, yf, scales=scales, workspace=ws)
+            bq.linear_static(x, params, pw, ys)
+    for xb in xs:
+        x.copy_(bf16_dev(xb))
+        graph.replay()
+        torch.cuda.synchronize()
+        ref = oracle.linear(xb, W["w_nibbles"], W["w_scale"], fb, 0.9, 1.0, None, b, 0)
+        assert np.array_equal(bits_host(yf), ref["y"])
+        assert np.array_equal(bits_host(ys), ref["y"])
+        assert np.array_equal(scales.cpu().numpy().view(np.uint32), ref["scales"].view(np.uint32))
+
+
 def test_fused_launches_overlapping_on_two_streams():
     # two fused launches in flight at once, each with its own workspace: neither fits the GPU next
     # to the other, so CTAs of both wait for SMs while resident ones wait for quantised rows --
